@@ -1,0 +1,147 @@
+/* purify_op.h - C ABI of the B200-native measurement operator  Phi = W G F Z S  and its adjoint.
+ *
+ * What it computes (arXiv 1903.04502, /root/reference/PAPER.md):
+ *   Eq. (2):  y = W G F Z S x  with S the gridding correction, Z zero padding
+ *   (oversampling factor 2), F a 2-D FFT on the K x K oversampled grid (K = 2n), G the
+ *   Kaiser-Bessel degridding onto M visibilities at continuous (u, v), W the noise weights;
+ *   the adjoint Phi^dagger "consists of applying these operators in reverse"
+ *   (S^dagger Z^dagger F^dagger G^dagger W^dagger).  Phi and Phi^dagger are applied once each per
+ *   ADMM iteration (Algorithm 1 lines 3 and 6).  The interpolation matrix G is
+ *   never stored (the thing PAPER.md:580-592 "Kernel Pre-Sampling" gets rid of): kernel weights are
+ *   evaluated on the fly (ANALYTIC) or read from the paper's pre-sampled table (TABLE).
+ *   Exact definitions, including every reading taken where the paper is silent: DESIGN.md.
+ *
+ * Conventions
+ *   image   x[py*n + px], interleaved complex (re, im), px fastest; px <-> u, py <-> v; the pixel
+ *           (n/2, n/2) is the phase centre.  n even.
+ *   (u, v)  uv[k][0] = u_k, uv[k][1] = v_k in OVERSAMPLED-GRID CELLS, DC at 0, period K = 2n
+ *           (paper's radians/pixel omega: u = omega K / 2 pi).  Any finite value with
+ *           |u| < 2^30 is accepted and taken mod K.
+ *   dtype   PURIFY_C64 : x, y complex64,  uv and w float32.   PURIFY_C128: complex128 / float64.
+ *   order   "caller order" = the order of uv at create.  "native order" = the library's tile-sorted
+ *           order; native[i] = caller[perm[i]] with perm from purify_op_permutation().
+ *   memory  "_dev" pointers are CUDA device pointers on the current device, "_host" pointers are
+ *           host pointers (pinned memory recommended).  The caller owns every buffer it passes; the
+ *           handle owns its sorted copies, tables, grid workspace and cuFFT plan.
+ *   stream  `cuda_stream` is a cudaStream_t cast to void* (NULL = legacy default stream).  All work
+ *           is enqueued on it; only purify_op_create*, the *_host calls (they return after the
+ *           result is in host memory) and purify_stage_times_ms synchronise.
+ *   errors  every function returns a purify_status (0 = OK, < 0 = error); nothing throws, aborts or
+ *           prints.  purify_last_error() gives a thread-local detail string for the last failure.
+ *   thread  a handle is not re-entrant (one workspace); distinct handles are independent.
+ *   determinism  degrid is bit-reproducible.  grid/normal flush partial tiles with floating-point
+ *           atomics, so the last bits of the gridded image may vary from call to call.
+ */
+#ifndef PURIFY_OP_H
+#define PURIFY_OP_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct purify_op purify_op; /* opaque */
+
+typedef enum { PURIFY_C64 = 0, PURIFY_C128 = 1 } purify_dtype;
+typedef enum { PURIFY_KERNEL_ANALYTIC = 0, PURIFY_KERNEL_TABLE = 1 } purify_kernel_mode;
+
+typedef enum {
+    PURIFY_OK = 0,
+    PURIFY_ERR_INVALID_ARG = -1, /* NULL pointer, n odd or <= 0, M < 0 or >= 2^31, J not in {4,6,8} */
+    PURIFY_ERR_UNSUPPORTED = -2, /* oversample != 2, unknown dtype / kernel mode                    */
+    PURIFY_ERR_UV_NONFINITE = -3,/* a NaN / Inf / |u| >= 2^30 coordinate was found at create        */
+    PURIFY_ERR_ALLOC = -4,       /* device or host allocation failed                                 */
+    PURIFY_ERR_CUDA = -5,        /* a CUDA runtime / driver call failed (detail in last_error)       */
+    PURIFY_ERR_CUFFT = -6,       /* a cuFFT call failed                                              */
+    PURIFY_ERR_NO_DEVICE = -7    /* no CUDA device: there is NO CPU fallback                         */
+} purify_status;
+
+/* Options; pass NULL for defaults.  Zero in any field means "default". */
+typedef struct {
+    int kernel_mode;            /* purify_kernel_mode; default ANALYTIC                              */
+    int table_samples_per_unit; /* TABLE mode: samples per grid cell R; default 4096
+                                   (BASELINE.json configs[4]); paper used 2e5.
+                                   T[i] = g(i/R), i = 0..R*J/2+1, lookup T[floor(|d| R + 1/2)].      */
+    int chunk;                  /* visibilities per work item (CTA); default 4096                    */
+    int time_stages;            /* != 0: record CUDA events around each stage                        */
+    int reserved[4];
+} purify_opts;
+
+/* Facts about a handle (for tests, benches and roofline arithmetic). */
+typedef struct {
+    int n, K, J, dtype, kernel_mode, table_samples_per_unit;
+    long long M;
+    int tile;                   /* tile side T in grid cells                                         */
+    int n_tiles;                /* tiles on the K x K grid                                           */
+    int n_tiles_nonempty;
+    int n_items;                /* work items (tile chunks) = CTAs per degrid / grid launch          */
+    int poly_degree;            /* ANALYTIC: degree of the per-tap polynomial in the cell offset     */
+    double poly_max_abs_err;    /* ANALYTIC: max |poly - g| over the support (fit check at create)   */
+    long long device_bytes;     /* device memory owned by the handle                                 */
+    long long max_tile_count;   /* visibilities in the fullest tile                                  */
+} purify_info;
+
+/* Stage indices for purify_stage_times_ms (milliseconds of the LAST call that ran the stage). */
+enum { PURIFY_STAGE_PAD = 0,   /* S + Z fused */
+       PURIFY_STAGE_FFT = 1,   /* F, cuFFT                         (a2)                */
+       PURIFY_STAGE_DEGRID = 2,/* W G                              (a3)                */
+       PURIFY_STAGE_GRID = 3,  /* G^dagger W^dagger incl. zeroing  (a4)                */
+       PURIFY_STAGE_IFFT = 4,  /* F^dagger, cuFFT                  (a5)                */
+       PURIFY_STAGE_CROP = 5,  /* Z^dagger S^dagger fused          (a6)                */
+       PURIFY_STAGE_PERMUTE = 6,
+       PURIFY_STAGE_COUNT = 8 };
+
+/* a0: build an operator for an n x n image, K = oversample*n, J-tap Kaiser-Bessel
+ * kernel (beta = 2.34 J) and M visibilities.  uv_dev: [M][2] (u, v); w_dev: [M] real weights or NULL
+ * (=> 1).  Copies uv and w (the caller may free them when this returns), bins the visibilities by
+ * grid tile (device radix sort on tile/cell id, once), builds the correction vector, the kernel
+ * polynomial or table and the cuFFT plan.  Synchronises the stream.  On error *out = NULL.         */
+int purify_op_create(purify_op **out, int n, int oversample, int J, long long M,
+                     const void *uv_dev, const void *w_dev, int dtype,
+                     const purify_opts *opts, void *cuda_stream);
+/* Same with uv / w in host memory. */
+int purify_op_create_host(purify_op **out, int n, int oversample, int J, long long M,
+                          const void *uv_host, const void *w_host, int dtype,
+                          const purify_opts *opts, void *cuda_stream);
+int purify_op_destroy(purify_op *op);
+int purify_op_info(const purify_op *op, purify_info *info);
+/* perm_dev[i] = caller index of the visibility at native position i (device pointer, M entries). */
+int purify_op_permutation(const purify_op *op, const unsigned **perm_dev);
+
+/* Phi (a1-a3):  x_dev[n*n] -> y_dev[M], caller order. */
+int purify_degrid(purify_op *op, const void *x_dev, void *y_dev, void *cuda_stream);
+/* Phi^dagger (a4-a6):  y_dev[M] (caller order) -> x_dev[n*n]. */
+int purify_grid(purify_op *op, const void *y_dev, void *x_dev, void *cuda_stream);
+/* Phi^dagger Phi (a7): x_in_dev -> x_out_dev (may alias); y stays in the handle's workspace. */
+int purify_normal(purify_op *op, const void *x_in_dev, void *x_out_dev, void *cuda_stream);
+
+/* Same operators with y in NATIVE order (moves only the minimum bytes; an ADMM loop can keep all
+ * its M-sized vectors in this order after one purify_permute_to_native of the data). */
+int purify_degrid_native(purify_op *op, const void *x_dev, void *y_native_dev, void *cuda_stream);
+int purify_grid_native(purify_op *op, const void *y_native_dev, void *x_dev, void *cuda_stream);
+int purify_permute_to_native(purify_op *op, const void *y_caller_dev, void *y_native_dev, void *cuda_stream);
+int purify_permute_from_native(purify_op *op, const void *y_native_dev, void *y_caller_dev, void *cuda_stream);
+
+/* Host-buffer entry points (end-to-end path): copy in, run, copy out, synchronise. */
+int purify_degrid_host(purify_op *op, const void *x_host, void *y_host, void *cuda_stream);
+int purify_grid_host(purify_op *op, const void *y_host, void *x_host, void *cuda_stream);
+int purify_normal_host(purify_op *op, const void *x_in_host, void *x_out_host, void *cuda_stream);
+
+/* Stage access for tests (device pointers): the K x K Fourier grid workspace in the library's
+ * internal layout is NOT exposed; these run single stages into caller buffers in the mathematical
+ * layout B[ky*K + kx], ky, kx in [0, K) (DC at index 0), so they can be compared with the oracle. */
+int purify_stage_fourier_grid(purify_op *op, const void *x_dev, void *B_dev /* K*K complex */, void *cuda_stream);
+int purify_stage_gridded(purify_op *op, const void *y_dev /* caller order */, void *B_dev, void *cuda_stream);
+
+/* Milliseconds per stage of the last call (needs opts.time_stages); synchronises. */
+int purify_stage_times_ms(const purify_op *op, float out[PURIFY_STAGE_COUNT]);
+/* Number of kernels of this library (cuFFT launches not counted) enqueued by the last call. */
+int purify_last_launch_count(const purify_op *op);
+
+const char *purify_strerror(int status);
+const char *purify_last_error(void);
+int purify_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PURIFY_OP_H */

@@ -1,0 +1,279 @@
+// Device kernels of the measurement operator (sm_100a).  DESIGN.md "Kernels" describes each one,
+// the roofline that bounds it and its algorithmic bytes per visibility.
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace pk {
+
+constexpr int TILE = 32;   // tile side in grid cells (T)
+
+template <typename R> struct Cplx;
+template <> struct Cplx<float> { typedef float2 type; };
+template <> struct Cplx<double> { typedef double2 type; };
+
+template <typename R> __device__ __forceinline__ typename Cplx<R>::type mk2(R a, R b);
+template <> __device__ __forceinline__ float2 mk2<float>(float a, float b) { return make_float2(a, b); }
+template <> __device__ __forceinline__ double2 mk2<double>(double a, double b) { return make_double2(a, b); }
+
+// Polynomial coefficients of the kernel taps (kb_host.hpp PolyFit), passed by value in the
+// kernel parameter (constant) bank so that Horner steps read them as immediate c[][] operands.
+template <typename R> struct KbCoef {
+    R e[4][9];
+    R o[4][9];
+};
+
+// One work item = one chunk of one tile's visibilities (native order range [start, start+count)).
+struct Item {
+    int x0, y0;      // tile origin in the internal (DC-centred) grid layout
+    int start, count;
+};
+
+template <typename R> struct OpParams {
+    typename Cplx<R>::type* grid;   // K*K internal layout: index (cy + K/2 mod K)*K + (cx + K/2 mod K)
+    int K, Kh, kmask;               // Kh = K/2; kmask = K-1 if K is a power of two else 0
+    const Item* items;
+    const typename Cplx<R>::type* uv;   // native order (u, v)
+    const R* w;                         // native order weights
+    const unsigned* perm;               // native -> caller index, or nullptr for native-order y
+    KbCoef<R> coef;
+    const R* table;                     // TABLE mode
+    R table_R;
+    int table_len;
+};
+
+__device__ __forceinline__ int wrap_idx(int a, int K, int kmask) {
+    if (kmask) return a & kmask;
+    int r = a % K;
+    return r < 0 ? r + K : r;
+}
+
+__device__ __forceinline__ float floor_r(float a) { return floorf(a); }
+__device__ __forceinline__ double floor_r(double a) { return floor(a); }
+__device__ __forceinline__ float sub_rn(float a, float b) { return __fsub_rn(a, b); }
+__device__ __forceinline__ double sub_rn(double a, double b) { return __dsub_rn(a, b); }
+__device__ __forceinline__ float mul_rn(float a, float b) { return __fmul_rn(a, b); }
+__device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ float add_rn(float a, float b) { return __fadd_rn(a, b); }
+__device__ __forceinline__ double add_rn(double a, double b) { return __dadd_rn(a, b); }
+__device__ __forceinline__ float fma_r(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ double fma_r(double a, double b, double c) { return fma(a, b, c); }
+
+// Kernel weights of the J taps c_j = cell - J/2 + 1 + j of one coordinate.
+//   ANALYTIC (MODE 0): per-tap-pair even/odd polynomials in t = (u - cell) - 1/2.
+//   TABLE    (MODE 1): T[floor(|u - c| R + 1/2)], each step one IEEE operation in R's precision
+//                      (reading R11; the oracle decides the index in the same precision).
+template <typename R, int J, int DEG, int MODE>
+__device__ __forceinline__ void kb_weights(R u, R cellf, int cell, const OpParams<R>& p, R (&g)[J]) {
+    if (MODE == 0) {
+        constexpr int NE = DEG / 2 + 1, NO = (DEG + 1) / 2;
+        const R t = (u - cellf) - (R)0.5;
+        const R t2 = t * t;
+#pragma unroll
+        for (int j = 0; j < J / 2; ++j) {
+            R E = p.coef.e[j][NE - 1], O = p.coef.o[j][NO - 1];
+#pragma unroll
+            for (int m = NE - 2; m >= 0; --m) E = fma_r(E, t2, p.coef.e[j][m]);
+#pragma unroll
+            for (int m = NO - 2; m >= 0; --m) O = fma_r(O, t2, p.coef.o[j][m]);
+            const R tO = t * O;
+            g[j] = E + tO;
+            g[J - 1 - j] = E - tO;
+        }
+    } else {
+#pragma unroll
+        for (int j = 0; j < J; ++j) {
+            const int c = cell - J / 2 + 1 + j;
+            const R d = sub_rn(u, (R)c);
+            const R a = mul_rn(fabs(d), p.table_R);
+            const R b = add_rn(a, (R)0.5);
+            const int idx = (int)floor_r(b);
+            g[j] = idx < p.table_len ? __ldg(p.table + idx) : (R)0;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// mbarrier / TMA helpers (inline PTX)
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void fence_barrier_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t phase) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(phase) : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* tmap, int x, int y, uint64_t* bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+        ::"r"(smem_u32(smem_dst)), "l"(tmap), "r"(x), "r"(y), "r"(smem_u32(bar)) : "memory");
+}
+
+// ---------------------------------------------------------------------------------------------
+// a1: S + Z fused.  Writes the WHOLE K x K grid: b[p^ mod K] = sign s[py] s[px] x[py,px], 0 elsewhere,
+// with sign = (-1)^(p^x + p^y) so that the FFT output lands DC-centred (index c + K/2): the dense
+// part of the uv plane is then in the interior of the grid and tiles there never wrap.
+// One thread per 16 bytes of grid (2 complex64 / 1 complex128), fully coalesced vector stores.
+template <typename R>
+__global__ void __launch_bounds__(256) pad_kernel(const typename Cplx<R>::type* __restrict__ x,
+                                                  const R* __restrict__ s, typename Cplx<R>::type* __restrict__ b,
+                                                  int n, int K) {
+    typedef typename Cplx<R>::type C;
+    constexpr int V = 16 / sizeof(C);           // complex elements per thread
+    const int vec_per_row = K / V;
+    const long long total = (long long)K * vec_per_row;
+    const int nh = n / 2;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total;
+         i += (long long)gridDim.x * blockDim.x) {
+        const int jy = (int)(i / vec_per_row);
+        const int jx0 = (int)(i % vec_per_row) * V;
+        const int py = jy < nh ? jy + nh : (jy >= K - nh ? jy - (K - nh) : -1);
+        C out[V];
+#pragma unroll
+        for (int e = 0; e < V; ++e) {
+            const int jx = jx0 + e;
+            const int px = jx < nh ? jx + nh : (jx >= K - nh ? jx - (K - nh) : -1);
+            if (py >= 0 && px >= 0) {
+                const C v = x[(long long)py * n + px];
+                R f = s[py] * s[px];
+                if ((jx + jy) & 1) f = -f;
+                out[e] = mk2<R>(f * v.x, f * v.y);
+            } else {
+                out[e] = mk2<R>((R)0, (R)0);
+            }
+        }
+        if constexpr (V == 2) {
+            reinterpret_cast<float4*>(b)[i] = make_float4(out[0].x, out[0].y, out[1].x, out[1].y);
+        } else {
+            b[i] = out[0];
+        }
+    }
+}
+
+// a6: Z^dagger S^dagger fused: x'[py,px] = sign s[py] s[px] b'[p^y mod K, p^x mod K].
+template <typename R>
+__global__ void __launch_bounds__(256) crop_kernel(const typename Cplx<R>::type* __restrict__ b,
+                                                   const R* __restrict__ s, typename Cplx<R>::type* __restrict__ x,
+                                                   int n, int K) {
+    typedef typename Cplx<R>::type C;
+    const int nh = n / 2;
+    const long long total = (long long)n * n;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total;
+         i += (long long)gridDim.x * blockDim.x) {
+        const int py = (int)(i / n), px = (int)(i % n);
+        const int jy = py >= nh ? py - nh : py + K - nh;
+        const int jx = px >= nh ? px - nh : px + K - nh;
+        const C v = b[(long long)jy * K + jx];
+        R f = s[py] * s[px];
+        if ((jx + jy) & 1) f = -f;
+        x[i] = mk2<R>(f * v.x, f * v.y);
+    }
+}
+
+// Internal (DC-centred) layout <-> mathematical layout B[ky*K+kx] (test/stage access only).
+template <typename R>
+__global__ void relayout_kernel(const typename Cplx<R>::type* __restrict__ in, typename Cplx<R>::type* __restrict__ out,
+                                int K, int to_math) {
+    const long long total = (long long)K * K;
+    const int Kh = K / 2;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total;
+         i += (long long)gridDim.x * blockDim.x) {
+        const int r = (int)(i / K), c = (int)(i % K);
+        const int r2 = (r + Kh) % K, c2 = (c + Kh) % K;      // K even: the shift is its own inverse
+        (void)to_math;
+        out[(long long)r2 * K + c2] = in[i];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a0: sort key per visibility: (tile, cell-in-tile), tile-major then row-major cell order.
+template <typename R>
+__global__ void key_kernel(const typename Cplx<R>::type* __restrict__ uv, long long M, int K, int kmask, int ntx,
+                           unsigned* __restrict__ keys, unsigned* __restrict__ idx, int* __restrict__ bad) {
+    for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < M; k += (long long)gridDim.x * blockDim.x) {
+        const typename Cplx<R>::type c = uv[k];
+        unsigned key = 0;
+        if (!(fabs(c.x) < (R)1073741824.0) || !(fabs(c.y) < (R)1073741824.0)) {   // NaN, Inf, too large
+            atomicOr(bad, 1);
+        } else {
+            const int gx = wrap_idx((int)floor_r(c.x) + K / 2, K, kmask);
+            const int gy = wrap_idx((int)floor_r(c.y) + K / 2, K, kmask);
+            const unsigned tile = (unsigned)(gy / TILE) * ntx + (unsigned)(gx / TILE);
+            key = (tile * TILE + (unsigned)(gy % TILE)) * TILE + (unsigned)(gx % TILE);
+        }
+        keys[k] = key;
+        idx[k] = (unsigned)k;
+    }
+}
+
+template <typename R>
+__global__ void gather_kernel(const typename Cplx<R>::type* __restrict__ uv, const R* __restrict__ w,
+                              const unsigned* __restrict__ perm, long long M,
+                              typename Cplx<R>::type* __restrict__ uv_s, R* __restrict__ w_s) {
+    for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < M; k += (long long)gridDim.x * blockDim.x) {
+        const unsigned src = perm[k];
+        uv_s[k] = uv[src];
+        w_s[k] = w ? w[src] : (R)1;
+    }
+}
+
+// tile_start[t] = first native index whose key >= t*TILE*TILE (binary search), t = 0..n_tiles.
+__global__ void tile_start_kernel(const unsigned* __restrict__ keys, long long M, int n_tiles, int* __restrict__ tile_start) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t > n_tiles) return;
+    const unsigned long long target = (unsigned long long)t * TILE * TILE;
+    long long lo = 0, hi = M;
+    while (lo < hi) {
+        const long long mid = (lo + hi) >> 1;
+        if ((unsigned long long)keys[mid] < target) lo = mid + 1; else hi = mid;
+    }
+    tile_start[t] = (int)lo;
+}
+
+__global__ void tile_chunks_kernel(const int* __restrict__ tile_start, int n_tiles, int chunk, int* __restrict__ n_chunks) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n_tiles) return;
+    const int cnt = tile_start[t + 1] - tile_start[t];
+    n_chunks[t] = (cnt + chunk - 1) / chunk;
+}
+
+__global__ void fill_items_kernel(const int* __restrict__ tile_start, const int* __restrict__ chunk_off, int n_tiles,
+                                  int ntx, int chunk, Item* __restrict__ items) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n_tiles) return;
+    const int s = tile_start[t], e = tile_start[t + 1];
+    int o = chunk_off[t];
+    for (int a = s; a < e; a += chunk) {
+        Item it;
+        it.x0 = (t % ntx) * TILE;
+        it.y0 = (t / ntx) * TILE;
+        it.start = a;
+        it.count = min(chunk, e - a);
+        items[o++] = it;
+    }
+}
+
+template <typename C>
+__global__ void permute_kernel(const C* __restrict__ in, C* __restrict__ out, const unsigned* __restrict__ perm,
+                               long long M, int to_native) {
+    for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < M; k += (long long)gridDim.x * blockDim.x) {
+        if (to_native) out[k] = in[perm[k]]; else out[perm[k]] = in[k];
+    }
+}
+
+}  // namespace pk

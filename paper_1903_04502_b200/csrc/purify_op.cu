@@ -1,0 +1,745 @@
+// C-ABI implementation of include/purify_op.h (sm_100a).  Host logic only: validation, create-time
+// binning, launches.  Every arithmetic step of the path runs in the kernels of kernels.cuh,
+// degrid.cuh, grid.cuh; the FFT stage is cuFFT (allowed by the north star, timed separately).
+// There is no CPU fallback: without a CUDA device every entry point returns PURIFY_ERR_NO_DEVICE.
+#include "../../include/purify_op.h"
+
+#include <cub/cub.cuh>
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <cufft.h>
+
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "degrid.cuh"
+#include "grid.cuh"
+#include "kb_host.hpp"
+#include "kernels.cuh"
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int status, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return status;
+}
+
+#define CK(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess)                                                                     \
+            return fail(e_ == cudaErrorMemoryAllocation ? PURIFY_ERR_ALLOC : PURIFY_ERR_CUDA,     \
+                        "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+    } while (0)
+#define CKFFT(call)                                                                                \
+    do {                                                                                           \
+        cufftResult r_ = (call);                                                                   \
+        if (r_ != CUFFT_SUCCESS)                                                                   \
+            return fail(PURIFY_ERR_CUFFT, "%s failed: cufftResult %d (%s:%d)", #call, (int)r_, __FILE__, __LINE__); \
+    } while (0)
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+int grid_for(long long work, int threads, int cap = 148 * 16) {
+    long long b = (work + threads - 1) / threads;
+    if (b < 1) b = 1;
+    if (b > cap) b = cap;
+    return (int)b;
+}
+
+// degree of the per-tap polynomial per (dtype, J): kb_host.hpp fit errors
+constexpr int deg_c64(int J) { return J == 4 ? 8 : 7; }
+constexpr int deg_c128(int J) { return J == 4 ? 17 : (J == 6 ? 16 : 15); }
+
+}  // namespace
+
+struct purify_op {
+    int n = 0, K = 0, J = 0, dtype = 0, mode = 0, table_R = 0, chunk = 4096, time_stages = 0;
+    long long M = 0;
+    int ntx = 0, n_tiles = 0, n_items = 0, n_tiles_nonempty = 0;
+    long long max_tile_count = 0;
+    int poly_degree = 0;
+    double poly_err = 0;
+    long long device_bytes = 0;
+    // device memory (owned)
+    void* grid = nullptr;     // K*K complex, internal layout
+    void* uv_s = nullptr;     // native-order (u, v)
+    void* w_s = nullptr;      // native-order weights
+    unsigned* perm = nullptr; // native -> caller
+    pk::Item* items = nullptr;
+    void* corr = nullptr;     // s[n]
+    void* table = nullptr;
+    int table_len = 0;
+    void* y_ws = nullptr;     // M complex (purify_normal / host paths), lazily allocated
+    void* x_ws = nullptr;     // n*n complex staging for host paths
+    void* y_ws2 = nullptr;    // caller-order staging for host paths
+    cufftHandle plan = 0;
+    bool plan_ok = false;
+    CUtensorMap tmap;
+    pk::KbCoef<float> coef32;
+    pk::KbCoef<double> coef64;
+    cudaEvent_t ev[2 * PURIFY_STAGE_COUNT];
+    bool ev_ok = false;
+    bool stage_ran[PURIFY_STAGE_COUNT];
+    int launches = 0;
+};
+
+namespace {
+
+size_t csize(const purify_op* op) { return op->dtype == PURIFY_C64 ? 8 : 16; }
+size_t rsize(const purify_op* op) { return op->dtype == PURIFY_C64 ? 4 : 8; }
+
+int dev_alloc(purify_op* op, void** p, size_t bytes) {
+    if (bytes == 0) bytes = 16;
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e != cudaSuccess) {
+        *p = nullptr;
+        cudaGetLastError();
+        return fail(PURIFY_ERR_ALLOC, "cudaMalloc(%zu bytes) failed: %s", bytes, cudaGetErrorString(e));
+    }
+    op->device_bytes += (long long)bytes;
+    return PURIFY_OK;
+}
+
+struct StageTimer {
+    purify_op* op; int stage; cudaStream_t st;
+    StageTimer(purify_op* o, int s, cudaStream_t t) : op(o), stage(s), st(t) {
+        if (op->time_stages && op->ev_ok) { cudaEventRecord(op->ev[2 * stage], st); op->stage_ran[stage] = true; }
+    }
+    ~StageTimer() { if (op->time_stages && op->ev_ok) cudaEventRecord(op->ev[2 * stage + 1], st); }
+};
+
+template <typename R> pk::OpParams<R> make_params(const purify_op* op, bool caller_order) {
+    pk::OpParams<R> p;
+    p.grid = (typename pk::Cplx<R>::type*)op->grid;
+    p.K = op->K; p.Kh = op->K / 2;
+    p.kmask = (op->K & (op->K - 1)) == 0 ? op->K - 1 : 0;
+    p.items = op->items;
+    p.uv = (const typename pk::Cplx<R>::type*)op->uv_s;
+    p.w = (const R*)op->w_s;
+    p.perm = caller_order ? op->perm : nullptr;
+    if (sizeof(R) == 4) memcpy(&p.coef, &op->coef32, sizeof(p.coef)); else memcpy(&p.coef, &op->coef64, sizeof(p.coef));
+    p.table = (const R*)op->table;
+    p.table_R = (R)op->table_R;
+    p.table_len = op->table_len;
+    return p;
+}
+
+// ------------------------------------------------------------------------------- launches
+template <typename R, int J, int DEG> int launch_degrid_t(purify_op* op, void* y, bool caller_order, cudaStream_t st) {
+    typedef typename pk::Cplx<R>::type C;
+    if (op->n_items == 0) return PURIFY_OK;
+    constexpr int BOX = pk::DegridCfg<J>::BOX;
+    const size_t smem = sizeof(C) * BOX * BOX + 16;
+    pk::OpParams<R> p = make_params<R>(op, caller_order);
+    if (op->mode == PURIFY_KERNEL_ANALYTIC) {
+        auto kern = pk::degrid_kernel<R, J, DEG, 0>;
+        CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        kern<<<op->n_items, pk::DegridCfg<J>::THREADS, smem, st>>>(op->tmap, p, (C*)y);
+    } else {
+        auto kern = pk::degrid_kernel<R, J, DEG, 1>;
+        CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        kern<<<op->n_items, pk::DegridCfg<J>::THREADS, smem, st>>>(op->tmap, p, (C*)y);
+    }
+    op->launches++;
+    CK(cudaGetLastError());
+    return PURIFY_OK;
+}
+
+template <typename R, int J, int DEG> int launch_grid_t(purify_op* op, const void* y, bool caller_order, cudaStream_t st) {
+    typedef typename pk::Cplx<R>::type C;
+    CK(cudaMemsetAsync(op->grid, 0, sizeof(C) * (size_t)op->K * op->K, st));
+    if (op->n_items == 0) return PURIFY_OK;
+    const size_t smem = pk::grid_smem_bytes<R, J>();
+    pk::OpParams<R> p = make_params<R>(op, caller_order);
+    if (op->mode == PURIFY_KERNEL_ANALYTIC) {
+        auto kern = pk::grid_kernel<R, J, DEG, 0>;
+        CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        kern<<<op->n_items, pk::GridCfg<J>::THREADS, smem, st>>>(p, (const C*)y);
+    } else {
+        auto kern = pk::grid_kernel<R, J, DEG, 1>;
+        CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        kern<<<op->n_items, pk::GridCfg<J>::THREADS, smem, st>>>(p, (const C*)y);
+    }
+    op->launches++;
+    CK(cudaGetLastError());
+    return PURIFY_OK;
+}
+
+int launch_degrid(purify_op* op, void* y, bool caller_order, cudaStream_t st) {
+    StageTimer t(op, PURIFY_STAGE_DEGRID, st);
+    if (op->dtype == PURIFY_C64) {
+        switch (op->J) {
+            case 4: return launch_degrid_t<float, 4, deg_c64(4)>(op, y, caller_order, st);
+            case 6: return launch_degrid_t<float, 6, deg_c64(6)>(op, y, caller_order, st);
+            default: return launch_degrid_t<float, 8, deg_c64(8)>(op, y, caller_order, st);
+        }
+    }
+    switch (op->J) {
+        case 4: return launch_degrid_t<double, 4, deg_c128(4)>(op, y, caller_order, st);
+        case 6: return launch_degrid_t<double, 6, deg_c128(6)>(op, y, caller_order, st);
+        default: return launch_degrid_t<double, 8, deg_c128(8)>(op, y, caller_order, st);
+    }
+}
+
+int launch_grid(purify_op* op, const void* y, bool caller_order, cudaStream_t st) {
+    StageTimer t(op, PURIFY_STAGE_GRID, st);
+    if (op->dtype == PURIFY_C64) {
+        switch (op->J) {
+            case 4: return launch_grid_t<float, 4, deg_c64(4)>(op, y, caller_order, st);
+            case 6: return launch_grid_t<float, 6, deg_c64(6)>(op, y, caller_order, st);
+            default: return launch_grid_t<float, 8, deg_c64(8)>(op, y, caller_order, st);
+        }
+    }
+    switch (op->J) {
+        case 4: return launch_grid_t<double, 4, deg_c128(4)>(op, y, caller_order, st);
+        case 6: return launch_grid_t<double, 6, deg_c128(6)>(op, y, caller_order, st);
+        default: return launch_grid_t<double, 8, deg_c128(8)>(op, y, caller_order, st);
+    }
+}
+
+int launch_pad(purify_op* op, const void* x, cudaStream_t st) {
+    StageTimer t(op, PURIFY_STAGE_PAD, st);
+    const long long vecs = (long long)op->K * op->K * (long long)csize(op) / 16;
+    if (op->dtype == PURIFY_C64)
+        pk::pad_kernel<float><<<grid_for(vecs, 256, 148 * 32), 256, 0, st>>>((const float2*)x, (const float*)op->corr,
+                                                                             (float2*)op->grid, op->n, op->K);
+    else
+        pk::pad_kernel<double><<<grid_for(vecs, 256, 148 * 32), 256, 0, st>>>((const double2*)x, (const double*)op->corr,
+                                                                              (double2*)op->grid, op->n, op->K);
+    op->launches++;
+    CK(cudaGetLastError());
+    return PURIFY_OK;
+}
+
+int launch_crop(purify_op* op, void* x, cudaStream_t st) {
+    StageTimer t(op, PURIFY_STAGE_CROP, st);
+    const long long tot = (long long)op->n * op->n;
+    if (op->dtype == PURIFY_C64)
+        pk::crop_kernel<float><<<grid_for(tot, 256, 148 * 32), 256, 0, st>>>((const float2*)op->grid, (const float*)op->corr,
+                                                                             (float2*)x, op->n, op->K);
+    else
+        pk::crop_kernel<double><<<grid_for(tot, 256, 148 * 32), 256, 0, st>>>((const double2*)op->grid, (const double*)op->corr,
+                                                                              (double2*)x, op->n, op->K);
+    op->launches++;
+    CK(cudaGetLastError());
+    return PURIFY_OK;
+}
+
+int launch_fft(purify_op* op, int dir, cudaStream_t st) {
+    StageTimer t(op, dir == CUFFT_FORWARD ? PURIFY_STAGE_FFT : PURIFY_STAGE_IFFT, st);
+    CKFFT(cufftSetStream(op->plan, st));
+    if (op->dtype == PURIFY_C64)
+        CKFFT(cufftExecC2C(op->plan, (cufftComplex*)op->grid, (cufftComplex*)op->grid, dir));
+    else
+        CKFFT(cufftExecZ2Z(op->plan, (cufftDoubleComplex*)op->grid, (cufftDoubleComplex*)op->grid, dir));
+    return PURIFY_OK;
+}
+
+int launch_permute(purify_op* op, const void* in, void* out, int to_native, cudaStream_t st) {
+    StageTimer t(op, PURIFY_STAGE_PERMUTE, st);
+    if (op->M == 0) return PURIFY_OK;
+    if (op->dtype == PURIFY_C64)
+        pk::permute_kernel<float2><<<grid_for(op->M, 256, 148 * 32), 256, 0, st>>>((const float2*)in, (float2*)out, op->perm, op->M, to_native);
+    else
+        pk::permute_kernel<double2><<<grid_for(op->M, 256, 148 * 32), 256, 0, st>>>((const double2*)in, (double2*)out, op->perm, op->M, to_native);
+    op->launches++;
+    CK(cudaGetLastError());
+    return PURIFY_OK;
+}
+
+int ensure_ws(purify_op* op, void** p, size_t bytes) {
+    if (*p) return PURIFY_OK;
+    return dev_alloc(op, p, bytes);
+}
+
+void begin_call(purify_op* op) {
+    op->launches = 0;
+    for (int i = 0; i < PURIFY_STAGE_COUNT; ++i) op->stage_ran[i] = false;
+}
+
+int check_device() {
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev <= 0) {
+        cudaGetLastError();
+        return fail(PURIFY_ERR_NO_DEVICE, "no CUDA device available (%s); this library has no CPU fallback",
+                    e != cudaSuccess ? cudaGetErrorString(e) : "device count 0");
+    }
+    return PURIFY_OK;
+}
+
+}  // namespace
+
+// =============================================================================== create
+namespace {
+
+template <typename R>
+int build_bins(purify_op* op, const void* uv_dev, const void* w_dev, cudaStream_t st) {
+    typedef typename pk::Cplx<R>::type C;
+    const long long M = op->M;
+    const int K = op->K;
+    const int kmask = (K & (K - 1)) == 0 ? K - 1 : 0;
+    op->ntx = (K + pk::TILE - 1) / pk::TILE;
+    op->n_tiles = op->ntx * op->ntx;
+
+    int rc;
+    if ((rc = dev_alloc(op, &op->uv_s, sizeof(C) * (size_t)M))) return rc;
+    if ((rc = dev_alloc(op, &op->w_s, sizeof(R) * (size_t)M))) return rc;
+    if ((rc = dev_alloc(op, (void**)&op->perm, sizeof(unsigned) * (size_t)M))) return rc;
+
+    // temporaries (freed before return)
+    unsigned *keys = nullptr, *keys2 = nullptr, *idx = nullptr;
+    int *bad = nullptr, *tile_start = nullptr, *n_chunks = nullptr, *chunk_off = nullptr;
+    void* cub_tmp = nullptr;
+    auto cleanup = [&]() {
+        cudaFree(keys); cudaFree(keys2); cudaFree(idx); cudaFree(bad);
+        cudaFree(tile_start); cudaFree(n_chunks); cudaFree(chunk_off); cudaFree(cub_tmp);
+    };
+#define CKC(call)                                                                                       \
+    do {                                                                                                \
+        cudaError_t e_ = (call);                                                                        \
+        if (e_ != cudaSuccess) {                                                                        \
+            cleanup();                                                                                  \
+            return fail(e_ == cudaErrorMemoryAllocation ? PURIFY_ERR_ALLOC : PURIFY_ERR_CUDA,          \
+                        "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__);    \
+        }                                                                                               \
+    } while (0)
+
+    const size_t Mz = M > 0 ? (size_t)M : 1;
+    CKC(cudaMalloc(&keys, sizeof(unsigned) * Mz));
+    CKC(cudaMalloc(&keys2, sizeof(unsigned) * Mz));
+    CKC(cudaMalloc(&idx, sizeof(unsigned) * Mz));
+    CKC(cudaMalloc(&bad, sizeof(int)));
+    CKC(cudaMalloc(&tile_start, sizeof(int) * (size_t)(op->n_tiles + 1)));
+    CKC(cudaMalloc(&n_chunks, sizeof(int) * (size_t)(op->n_tiles + 1)));
+    CKC(cudaMalloc(&chunk_off, sizeof(int) * (size_t)(op->n_tiles + 1)));
+    CKC(cudaMemsetAsync(bad, 0, sizeof(int), st));
+    CKC(cudaMemsetAsync(n_chunks, 0, sizeof(int) * (size_t)(op->n_tiles + 1), st));
+
+    if (M > 0) {
+        pk::key_kernel<R><<<grid_for(M, 256), 256, 0, st>>>((const C*)uv_dev, M, K, kmask, op->ntx, keys, idx, bad);
+        CKC(cudaGetLastError());
+        int h_bad = 0;
+        CKC(cudaMemcpyAsync(&h_bad, bad, sizeof(int), cudaMemcpyDeviceToHost, st));
+        CKC(cudaStreamSynchronize(st));
+        if (h_bad) {
+            cleanup();
+            return fail(PURIFY_ERR_UV_NONFINITE, "uv contains NaN, Inf or |coordinate| >= 2^30");
+        }
+        // device radix sort on (tile, cell) id; only the significant key bits are sorted
+        int bits = 1;
+        while (bits < 32 && (1ull << bits) < (unsigned long long)op->n_tiles * pk::TILE * pk::TILE) ++bits;
+        size_t tmp_bytes = 0;
+        CKC(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys, keys2, idx, op->perm, (int)M, 0, bits, st));
+        CKC(cudaMalloc(&cub_tmp, tmp_bytes ? tmp_bytes : 16));
+        CKC(cub::DeviceRadixSort::SortPairs(cub_tmp, tmp_bytes, keys, keys2, idx, op->perm, (int)M, 0, bits, st));
+        pk::gather_kernel<R><<<grid_for(M, 256), 256, 0, st>>>((const C*)uv_dev, (const R*)w_dev, op->perm, M,
+                                                                (C*)op->uv_s, (R*)op->w_s);
+        CKC(cudaGetLastError());
+    }
+    pk::tile_start_kernel<<<(op->n_tiles + 1 + 255) / 256, 256, 0, st>>>(keys2, M, op->n_tiles, tile_start);
+    CKC(cudaGetLastError());
+    pk::tile_chunks_kernel<<<(op->n_tiles + 255) / 256, 256, 0, st>>>(tile_start, op->n_tiles, op->chunk, n_chunks);
+    CKC(cudaGetLastError());
+    {
+        size_t tmp2 = 0;
+        void* t2 = nullptr;
+        CKC(cub::DeviceScan::ExclusiveSum(nullptr, tmp2, n_chunks, chunk_off, op->n_tiles + 1, st));
+        CKC(cudaMalloc(&t2, tmp2 ? tmp2 : 16));
+        cudaError_t e2 = cub::DeviceScan::ExclusiveSum(t2, tmp2, n_chunks, chunk_off, op->n_tiles + 1, st);
+        cudaError_t e3 = cudaStreamSynchronize(st);
+        cudaFree(t2);
+        CKC(e2);
+        CKC(e3);
+    }
+    CKC(cudaMemcpy(&op->n_items, chunk_off + op->n_tiles, sizeof(int), cudaMemcpyDeviceToHost));
+    // tile statistics (host side; n_tiles is small)
+    {
+        std::vector<int> ts((size_t)op->n_tiles + 1);
+        CKC(cudaMemcpy(ts.data(), tile_start, sizeof(int) * ts.size(), cudaMemcpyDeviceToHost));
+        op->n_tiles_nonempty = 0;
+        op->max_tile_count = 0;
+        for (int t = 0; t < op->n_tiles; ++t) {
+            const int c = ts[t + 1] - ts[t];
+            if (c > 0) op->n_tiles_nonempty++;
+            if (c > op->max_tile_count) op->max_tile_count = c;
+        }
+    }
+    {
+        void* items = nullptr;
+        cudaError_t e = cudaMalloc(&items, sizeof(pk::Item) * (size_t)(op->n_items > 0 ? op->n_items : 1));
+        if (e != cudaSuccess) { cleanup(); cudaGetLastError(); return fail(PURIFY_ERR_ALLOC, "cudaMalloc(items) failed"); }
+        op->items = (pk::Item*)items;
+        op->device_bytes += (long long)sizeof(pk::Item) * (op->n_items > 0 ? op->n_items : 1);
+    }
+    if (op->n_items > 0) {
+        pk::fill_items_kernel<<<(op->n_tiles + 255) / 256, 256, 0, st>>>(tile_start, chunk_off, op->n_tiles, op->ntx,
+                                                                         op->chunk, op->items);
+        CKC(cudaGetLastError());
+    }
+    CKC(cudaStreamSynchronize(st));
+    cleanup();
+#undef CKC
+    return PURIFY_OK;
+}
+
+template <typename R>
+int build_tables(purify_op* op, cudaStream_t st) {
+    int rc;
+    // gridding correction s[n]
+    std::vector<double> s;
+    kbhost::correction(op->n, op->J, s);
+    std::vector<R> sr(s.begin(), s.end());
+    if ((rc = dev_alloc(op, &op->corr, sizeof(R) * (size_t)op->n))) return rc;
+    CK(cudaMemcpyAsync(op->corr, sr.data(), sizeof(R) * (size_t)op->n, cudaMemcpyHostToDevice, st));
+    CK(cudaStreamSynchronize(st));
+    // kernel polynomial
+    kbhost::PolyFit fit;
+    const int deg = sizeof(R) == 4 ? deg_c64(op->J) : deg_c128(op->J);
+    kbhost::fit_poly(op->J, deg, fit);
+    op->poly_degree = deg;
+    op->poly_err = fit.max_abs_err;
+    for (int j = 0; j < 4; ++j)
+        for (int m = 0; m < 9; ++m) {
+            op->coef32.e[j][m] = (float)fit.e[j][m]; op->coef32.o[j][m] = (float)fit.o[j][m];
+            op->coef64.e[j][m] = fit.e[j][m];        op->coef64.o[j][m] = fit.o[j][m];
+        }
+    // pre-sampled table
+    if (op->mode == PURIFY_KERNEL_TABLE) {
+        std::vector<double> T;
+        kbhost::table(op->J, op->table_R, T);
+        std::vector<R> Tr(T.begin(), T.end());
+        op->table_len = (int)Tr.size();
+        if ((rc = dev_alloc(op, &op->table, sizeof(R) * Tr.size()))) return rc;
+        CK(cudaMemcpyAsync(op->table, Tr.data(), sizeof(R) * Tr.size(), cudaMemcpyHostToDevice, st));
+        CK(cudaStreamSynchronize(st));
+    }
+    return PURIFY_OK;
+}
+
+int build_tmap(purify_op* op) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    CK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+    if (!fn || qres != cudaDriverEntryPointSuccess)
+        return fail(PURIFY_ERR_CUDA, "cuTensorMapEncodeTiled entry point not available");
+    const int BOX = pk::TILE + op->J;
+    const bool f32 = op->dtype == PURIFY_C64;
+    const cuuint64_t dims[2] = {(cuuint64_t)2 * op->K, (cuuint64_t)op->K};            // inner extent in reals
+    const cuuint64_t strides[1] = {(cuuint64_t)op->K * csize(op)};                     // row pitch, bytes
+    const cuuint32_t box[2] = {(cuuint32_t)(2 * BOX), (cuuint32_t)BOX};
+    const cuuint32_t estr[2] = {1, 1};
+    CUresult r = ((EncodeTiledFn)fn)(&op->tmap, f32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64,
+                                     2, op->grid, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                     CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(PURIFY_ERR_CUDA, "cuTensorMapEncodeTiled failed: CUresult %d", (int)r);
+    return PURIFY_OK;
+}
+
+int create_impl(purify_op** out, int n, int oversample, int J, long long M, const void* uv, const void* w,
+                bool host_inputs, int dtype, const purify_opts* opts, void* stream) {
+    if (!out) return fail(PURIFY_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (n <= 0 || (n & 1)) return fail(PURIFY_ERR_INVALID_ARG, "n must be positive and even (got %d)", n);
+    if (n > 16384) return fail(PURIFY_ERR_INVALID_ARG, "n too large (got %d, max 16384)", n);
+    if (oversample != 2) return fail(PURIFY_ERR_UNSUPPORTED, "only oversample = 2 is supported (got %d)", oversample);
+    if (J != 4 && J != 6 && J != 8) return fail(PURIFY_ERR_INVALID_ARG, "J must be 4, 6 or 8 (got %d)", J);
+    if (M < 0 || M >= (1ll << 31)) return fail(PURIFY_ERR_INVALID_ARG, "M must be in [0, 2^31) (got %lld)", M);
+    if (M > 0 && !uv) return fail(PURIFY_ERR_INVALID_ARG, "uv is NULL");
+    if (dtype != PURIFY_C64 && dtype != PURIFY_C128) return fail(PURIFY_ERR_UNSUPPORTED, "unknown dtype %d", dtype);
+    int mode = PURIFY_KERNEL_ANALYTIC, R = 4096, chunk = 4096, time_stages = 0;
+    if (opts) {
+        mode = opts->kernel_mode;
+        if (opts->table_samples_per_unit) R = opts->table_samples_per_unit;
+        if (opts->chunk) chunk = opts->chunk;
+        time_stages = opts->time_stages;
+    }
+    if (mode != PURIFY_KERNEL_ANALYTIC && mode != PURIFY_KERNEL_TABLE)
+        return fail(PURIFY_ERR_UNSUPPORTED, "unknown kernel mode %d", mode);
+    if (R < 1 || (long long)R * J / 2 + 2 > (1ll << 30)) return fail(PURIFY_ERR_INVALID_ARG, "bad table density %d", R);
+    if (chunk < 32 || chunk > (1 << 24)) return fail(PURIFY_ERR_INVALID_ARG, "chunk must be in [32, 2^24] (got %d)", chunk);
+    int rc = check_device();
+    if (rc) return rc;
+
+    purify_op* op = new (std::nothrow) purify_op();
+    if (!op) return fail(PURIFY_ERR_ALLOC, "host allocation failed");
+    op->n = n; op->K = 2 * n; op->J = J; op->M = M; op->dtype = dtype; op->mode = mode; op->table_R = R;
+    op->chunk = chunk; op->time_stages = time_stages;
+    cudaStream_t st = (cudaStream_t)stream;
+
+    void *uv_tmp = nullptr, *w_tmp = nullptr;
+    auto bail = [&](int code) { cudaFree(uv_tmp); cudaFree(w_tmp); purify_op_destroy(op); return code; };
+
+    const void *uv_dev = uv, *w_dev = w;
+    if (host_inputs && M > 0) {
+        const size_t ub = csize(op) * (size_t)M, wb = rsize(op) * (size_t)M;
+        if (cudaMalloc(&uv_tmp, ub) != cudaSuccess) { cudaGetLastError(); return bail(fail(PURIFY_ERR_ALLOC, "cudaMalloc(uv) failed")); }
+        if (cudaMemcpyAsync(uv_tmp, uv, ub, cudaMemcpyHostToDevice, st) != cudaSuccess) return bail(fail(PURIFY_ERR_CUDA, "H2D copy of uv failed"));
+        uv_dev = uv_tmp;
+        if (w) {
+            if (cudaMalloc(&w_tmp, wb) != cudaSuccess) { cudaGetLastError(); return bail(fail(PURIFY_ERR_ALLOC, "cudaMalloc(w) failed")); }
+            if (cudaMemcpyAsync(w_tmp, w, wb, cudaMemcpyHostToDevice, st) != cudaSuccess) return bail(fail(PURIFY_ERR_CUDA, "H2D copy of w failed"));
+            w_dev = w_tmp;
+        }
+    }
+
+    rc = dev_alloc(op, &op->grid, csize(op) * (size_t)op->K * op->K);
+    if (rc) return bail(rc);
+    rc = dtype == PURIFY_C64 ? build_bins<float>(op, uv_dev, w_dev, st) : build_bins<double>(op, uv_dev, w_dev, st);
+    if (rc) return bail(rc);
+    rc = dtype == PURIFY_C64 ? build_tables<float>(op, st) : build_tables<double>(op, st);
+    if (rc) return bail(rc);
+    rc = build_tmap(op);
+    if (rc) return bail(rc);
+    {
+        cufftResult r = cufftPlan2d(&op->plan, op->K, op->K, dtype == PURIFY_C64 ? CUFFT_C2C : CUFFT_Z2Z);
+        if (r != CUFFT_SUCCESS) return bail(fail(r == CUFFT_ALLOC_FAILED ? PURIFY_ERR_ALLOC : PURIFY_ERR_CUFFT,
+                                                 "cufftPlan2d(%d x %d) failed: cufftResult %d", op->K, op->K, (int)r));
+        op->plan_ok = true;
+        size_t ws = 0;
+        if (cufftGetSize(op->plan, &ws) == CUFFT_SUCCESS) op->device_bytes += (long long)ws;
+    }
+    for (int i = 0; i < 2 * PURIFY_STAGE_COUNT; ++i) {
+        if (cudaEventCreate(&op->ev[i]) != cudaSuccess) return bail(fail(PURIFY_ERR_CUDA, "cudaEventCreate failed"));
+    }
+    op->ev_ok = true;
+    begin_call(op);
+    if (cudaStreamSynchronize(st) != cudaSuccess) return bail(fail(PURIFY_ERR_CUDA, "stream synchronise failed in create"));
+    cudaFree(uv_tmp);
+    cudaFree(w_tmp);
+    *out = op;
+    return PURIFY_OK;
+}
+
+}  // namespace
+
+// =============================================================================== C ABI
+#define NEED_OP(op)                                                                 \
+    do {                                                                            \
+        if (!(op)) return fail(PURIFY_ERR_INVALID_ARG, "op is NULL");               \
+    } while (0)
+#define NEED_PTR(p, name)                                                           \
+    do {                                                                            \
+        if (!(p)) return fail(PURIFY_ERR_INVALID_ARG, name " is NULL");             \
+    } while (0)
+#define RUN(expr)                 \
+    do {                          \
+        int rc_ = (expr);         \
+        if (rc_) return rc_;      \
+    } while (0)
+
+extern "C" {
+
+int purify_op_create(purify_op** out, int n, int oversample, int J, long long M, const void* uv_dev,
+                     const void* w_dev, int dtype, const purify_opts* opts, void* cuda_stream) {
+    return create_impl(out, n, oversample, J, M, uv_dev, w_dev, false, dtype, opts, cuda_stream);
+}
+
+int purify_op_create_host(purify_op** out, int n, int oversample, int J, long long M, const void* uv_host,
+                          const void* w_host, int dtype, const purify_opts* opts, void* cuda_stream) {
+    return create_impl(out, n, oversample, J, M, uv_host, w_host, true, dtype, opts, cuda_stream);
+}
+
+int purify_op_destroy(purify_op* op) {
+    if (!op) return PURIFY_OK;
+    cudaFree(op->grid); cudaFree(op->uv_s); cudaFree(op->w_s); cudaFree(op->perm); cudaFree(op->items);
+    cudaFree(op->corr); cudaFree(op->table); cudaFree(op->y_ws); cudaFree(op->x_ws); cudaFree(op->y_ws2);
+    if (op->plan_ok) cufftDestroy(op->plan);
+    if (op->ev_ok) for (int i = 0; i < 2 * PURIFY_STAGE_COUNT; ++i) cudaEventDestroy(op->ev[i]);
+    cudaGetLastError();
+    delete op;
+    return PURIFY_OK;
+}
+
+int purify_op_info(const purify_op* op, purify_info* info) {
+    NEED_OP(op);
+    NEED_PTR(info, "info");
+    info->n = op->n; info->K = op->K; info->J = op->J; info->dtype = op->dtype; info->kernel_mode = op->mode;
+    info->table_samples_per_unit = op->table_R; info->M = op->M; info->tile = pk::TILE; info->n_tiles = op->n_tiles;
+    info->n_tiles_nonempty = op->n_tiles_nonempty; info->n_items = op->n_items; info->poly_degree = op->poly_degree;
+    info->poly_max_abs_err = op->poly_err; info->device_bytes = op->device_bytes; info->max_tile_count = op->max_tile_count;
+    return PURIFY_OK;
+}
+
+int purify_op_permutation(const purify_op* op, const unsigned** perm_dev) {
+    NEED_OP(op);
+    NEED_PTR(perm_dev, "perm_dev");
+    *perm_dev = op->perm;
+    return PURIFY_OK;
+}
+
+static int degrid_impl(purify_op* op, const void* x, void* y, bool caller_order, cudaStream_t st) {
+    RUN(launch_pad(op, x, st));
+    RUN(launch_fft(op, CUFFT_FORWARD, st));
+    RUN(launch_degrid(op, y, caller_order, st));
+    return PURIFY_OK;
+}
+
+static int grid_impl(purify_op* op, const void* y, void* x, bool caller_order, cudaStream_t st) {
+    RUN(launch_grid(op, y, caller_order, st));
+    RUN(launch_fft(op, CUFFT_INVERSE, st));
+    RUN(launch_crop(op, x, st));
+    return PURIFY_OK;
+}
+
+int purify_degrid(purify_op* op, const void* x_dev, void* y_dev, void* cuda_stream) {
+    NEED_OP(op); NEED_PTR(x_dev, "x"); if (op->M > 0) NEED_PTR(y_dev, "y");
+    begin_call(op);
+    return degrid_impl(op, x_dev, y_dev, true, (cudaStream_t)cuda_stream);
+}
+
+int purify_degrid_native(purify_op* op, const void* x_dev, void* y_native_dev, void* cuda_stream) {
+    NEED_OP(op); NEED_PTR(x_dev, "x"); if (op->M > 0) NEED_PTR(y_native_dev, "y");
+    begin_call(op);
+    return degrid_impl(op, x_dev, y_native_dev, false, (cudaStream_t)cuda_stream);
+}
+
+int purify_grid(purify_op* op, const void* y_dev, void* x_dev, void* cuda_stream) {
+    NEED_OP(op); NEED_PTR(x_dev, "x"); if (op->M > 0) NEED_PTR(y_dev, "y");
+    begin_call(op);
+    return grid_impl(op, y_dev, x_dev, true, (cudaStream_t)cuda_stream);
+}
+
+int purify_grid_native(purify_op* op, const void* y_native_dev, void* x_dev, void* cuda_stream) {
+    NEED_OP(op); NEED_PTR(x_dev, "x"); if (op->M > 0) NEED_PTR(y_native_dev, "y");
+    begin_call(op);
+    return grid_impl(op, y_native_dev, x_dev, false, (cudaStream_t)cuda_stream);
+}
+
+int purify_normal(purify_op* op, const void* x_in_dev, void* x_out_dev, void* cuda_stream) {
+    NEED_OP(op); NEED_PTR(x_in_dev, "x_in"); NEED_PTR(x_out_dev, "x_out");
+    begin_call(op);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    RUN(ensure_ws(op, &op->y_ws, csize(op) * (size_t)op->M));
+    RUN(degrid_impl(op, x_in_dev, op->y_ws, false, st));
+    RUN(grid_impl(op, op->y_ws, x_out_dev, false, st));
+    return PURIFY_OK;
+}
+
+int purify_permute_to_native(purify_op* op, const void* y_caller_dev, void* y_native_dev, void* cuda_stream) {
+    NEED_OP(op); if (op->M > 0) { NEED_PTR(y_caller_dev, "y_caller"); NEED_PTR(y_native_dev, "y_native"); }
+    begin_call(op);
+    return launch_permute(op, y_caller_dev, y_native_dev, 1, (cudaStream_t)cuda_stream);
+}
+
+int purify_permute_from_native(purify_op* op, const void* y_native_dev, void* y_caller_dev, void* cuda_stream) {
+    NEED_OP(op); if (op->M > 0) { NEED_PTR(y_caller_dev, "y_caller"); NEED_PTR(y_native_dev, "y_native"); }
+    begin_call(op);
+    return launch_permute(op, y_native_dev, y_caller_dev, 0, (cudaStream_t)cuda_stream);
+}
+
+// ---- host-buffer entry points (end-to-end path: H2D + operator + D2H inside the call)
+int purify_degrid_host(purify_op* op, const void* x_host, void* y_host, void* cuda_stream) {
+    NEED_OP(op); NEED_PTR(x_host, "x"); if (op->M > 0) NEED_PTR(y_host, "y");
+    begin_call(op);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t xb = csize(op) * (size_t)op->n * op->n, yb = csize(op) * (size_t)op->M;
+    RUN(ensure_ws(op, &op->x_ws, xb));
+    RUN(ensure_ws(op, &op->y_ws2, yb));
+    CK(cudaMemcpyAsync(op->x_ws, x_host, xb, cudaMemcpyHostToDevice, st));
+    RUN(degrid_impl(op, op->x_ws, op->y_ws2, true, st));
+    if (yb) CK(cudaMemcpyAsync(y_host, op->y_ws2, yb, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return PURIFY_OK;
+}
+
+int purify_grid_host(purify_op* op, const void* y_host, void* x_host, void* cuda_stream) {
+    NEED_OP(op); NEED_PTR(x_host, "x"); if (op->M > 0) NEED_PTR(y_host, "y");
+    begin_call(op);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t xb = csize(op) * (size_t)op->n * op->n, yb = csize(op) * (size_t)op->M;
+    RUN(ensure_ws(op, &op->x_ws, xb));
+    RUN(ensure_ws(op, &op->y_ws2, yb));
+    if (yb) CK(cudaMemcpyAsync(op->y_ws2, y_host, yb, cudaMemcpyHostToDevice, st));
+    RUN(grid_impl(op, op->y_ws2, op->x_ws, true, st));
+    CK(cudaMemcpyAsync(x_host, op->x_ws, xb, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return PURIFY_OK;
+}
+
+int purify_normal_host(purify_op* op, const void* x_in_host, void* x_out_host, void* cuda_stream) {
+    NEED_OP(op); NEED_PTR(x_in_host, "x_in"); NEED_PTR(x_out_host, "x_out");
+    begin_call(op);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t xb = csize(op) * (size_t)op->n * op->n;
+    RUN(ensure_ws(op, &op->x_ws, xb));
+    RUN(ensure_ws(op, &op->y_ws, csize(op) * (size_t)op->M));
+    CK(cudaMemcpyAsync(op->x_ws, x_in_host, xb, cudaMemcpyHostToDevice, st));
+    RUN(degrid_impl(op, op->x_ws, op->y_ws, false, st));
+    RUN(grid_impl(op, op->y_ws, op->x_ws, false, st));
+    CK(cudaMemcpyAsync(x_out_host, op->x_ws, xb, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return PURIFY_OK;
+}
+
+// ---- single stages in the mathematical layout (tests)
+static int relayout(purify_op* op, const void* in, void* out, cudaStream_t st) {
+    const long long tot = (long long)op->K * op->K;
+    if (op->dtype == PURIFY_C64)
+        pk::relayout_kernel<float><<<grid_for(tot, 256, 148 * 32), 256, 0, st>>>((const float2*)in, (float2*)out, op->K, 1);
+    else
+        pk::relayout_kernel<double><<<grid_for(tot, 256, 148 * 32), 256, 0, st>>>((const double2*)in, (double2*)out, op->K, 1);
+    op->launches++;
+    CK(cudaGetLastError());
+    return PURIFY_OK;
+}
+
+int purify_stage_fourier_grid(purify_op* op, const void* x_dev, void* B_dev, void* cuda_stream) {
+    NEED_OP(op); NEED_PTR(x_dev, "x"); NEED_PTR(B_dev, "B");
+    begin_call(op);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    RUN(launch_pad(op, x_dev, st));
+    RUN(launch_fft(op, CUFFT_FORWARD, st));
+    return relayout(op, op->grid, B_dev, st);
+}
+
+int purify_stage_gridded(purify_op* op, const void* y_dev, void* B_dev, void* cuda_stream) {
+    NEED_OP(op); NEED_PTR(B_dev, "B"); if (op->M > 0) NEED_PTR(y_dev, "y");
+    begin_call(op);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    RUN(launch_grid(op, y_dev, true, st));
+    return relayout(op, op->grid, B_dev, st);
+}
+
+int purify_stage_times_ms(const purify_op* op, float out[PURIFY_STAGE_COUNT]) {
+    NEED_OP(op); NEED_PTR(out, "out");
+    for (int i = 0; i < PURIFY_STAGE_COUNT; ++i) out[i] = 0.f;
+    if (!op->time_stages || !op->ev_ok) return fail(PURIFY_ERR_INVALID_ARG, "handle was created without opts.time_stages");
+    CK(cudaDeviceSynchronize());
+    for (int i = 0; i < PURIFY_STAGE_COUNT; ++i)
+        if (op->stage_ran[i]) CK(cudaEventElapsedTime(&out[i], op->ev[2 * i], op->ev[2 * i + 1]));
+    return PURIFY_OK;
+}
+
+int purify_last_launch_count(const purify_op* op) { return op ? op->launches : 0; }
+
+const char* purify_strerror(int status) {
+    switch (status) {
+        case PURIFY_OK: return "ok";
+        case PURIFY_ERR_INVALID_ARG: return "invalid argument";
+        case PURIFY_ERR_UNSUPPORTED: return "unsupported configuration";
+        case PURIFY_ERR_UV_NONFINITE: return "non-finite or out-of-range (u, v) coordinate";
+        case PURIFY_ERR_ALLOC: return "allocation failed";
+        case PURIFY_ERR_CUDA: return "CUDA error";
+        case PURIFY_ERR_CUFFT: return "cuFFT error";
+        case PURIFY_ERR_NO_DEVICE: return "no CUDA device (no CPU fallback)";
+        default: return "unknown status";
+    }
+}
+
+const char* purify_last_error(void) { return g_err; }
+int purify_version(void) { return 100; }
+
+}  // extern "C"

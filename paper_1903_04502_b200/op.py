@@ -1,0 +1,258 @@
+"""Thin Python binding of include/purify_op.h (ctypes).  Argument marshalling only: every step of
+the path runs in the CUDA library (csrc/).  PyTorch provides device memory and streams.
+
+There is NO CPU fallback: if libpurify_op.so is missing or there is no CUDA device, calls raise.
+This module never imports oracle/.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpurify_op.so")
+
+C64, C128 = 0, 1
+ANALYTIC, TABLE = 0, 1
+STAGES = ("pad", "fft", "degrid", "grid", "ifft", "crop", "permute", "reserved")
+
+# every symbol include/purify_op.h declares (checked by tests/test_abi.py)
+SYMBOLS = (
+    "purify_op_create", "purify_op_create_host", "purify_op_destroy", "purify_op_info",
+    "purify_op_permutation", "purify_degrid", "purify_grid", "purify_normal",
+    "purify_degrid_native", "purify_grid_native", "purify_permute_to_native",
+    "purify_permute_from_native", "purify_degrid_host", "purify_grid_host", "purify_normal_host",
+    "purify_stage_fourier_grid", "purify_stage_gridded", "purify_stage_times_ms",
+    "purify_last_launch_count", "purify_strerror", "purify_last_error", "purify_version",
+)
+
+
+class PurifyOpts(C.Structure):
+    _fields_ = [("kernel_mode", C.c_int), ("table_samples_per_unit", C.c_int), ("chunk", C.c_int),
+                ("time_stages", C.c_int), ("reserved", C.c_int * 4)]
+
+
+class PurifyInfo(C.Structure):
+    _fields_ = [("n", C.c_int), ("K", C.c_int), ("J", C.c_int), ("dtype", C.c_int), ("kernel_mode", C.c_int),
+                ("table_samples_per_unit", C.c_int), ("M", C.c_longlong), ("tile", C.c_int), ("n_tiles", C.c_int),
+                ("n_tiles_nonempty", C.c_int), ("n_items", C.c_int), ("poly_degree", C.c_int),
+                ("poly_max_abs_err", C.c_double), ("device_bytes", C.c_longlong), ("max_tile_count", C.c_longlong)]
+
+
+class PurifyError(RuntimeError):
+    def __init__(self, status: int, what: str, detail: str):
+        super().__init__(f"{what}: status {status} ({detail})")
+        self.status = status
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen the C-ABI library and declare its signatures.  Fails loudly if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise FileNotFoundError(
+            f"{LIB_PATH} not found: build it with `python -m paper_1903_04502_b200.build` "
+            "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    vp, ip, ll = C.c_void_p, C.c_int, C.c_longlong
+    L.purify_op_create.argtypes = [C.POINTER(vp), ip, ip, ip, ll, vp, vp, ip, C.POINTER(PurifyOpts), vp]
+    L.purify_op_create_host.argtypes = L.purify_op_create.argtypes
+    L.purify_op_destroy.argtypes = [vp]
+    L.purify_op_info.argtypes = [vp, C.POINTER(PurifyInfo)]
+    L.purify_op_permutation.argtypes = [vp, C.POINTER(vp)]
+    for name in ("purify_degrid", "purify_grid", "purify_normal", "purify_degrid_native", "purify_grid_native",
+                 "purify_permute_to_native", "purify_permute_from_native", "purify_degrid_host",
+                 "purify_grid_host", "purify_normal_host", "purify_stage_fourier_grid", "purify_stage_gridded"):
+        getattr(L, name).argtypes = [vp, vp, vp, vp]
+        getattr(L, name).restype = ip
+    L.purify_stage_times_ms.argtypes = [vp, C.POINTER(C.c_float)]
+    L.purify_last_launch_count.argtypes = [vp]
+    L.purify_strerror.argtypes = [ip]
+    L.purify_strerror.restype = C.c_char_p
+    L.purify_last_error.restype = C.c_char_p
+    L.purify_version.restype = ip
+    _lib = L
+    return L
+
+
+def _check(status: int, what: str):
+    if status != 0:
+        L = load_library()
+        raise PurifyError(status, what, f"{L.purify_strerror(status).decode()}: {L.purify_last_error().decode()}")
+
+
+def _stream() -> C.c_void_p:
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+_CDT = {C64: torch.complex64, C128: torch.complex128}
+_RDT = {C64: torch.float32, C128: torch.float64}
+
+
+class PurifyOp:
+    """Handle of one measurement operator (purify_op_create ... purify_op_destroy)."""
+
+    def __init__(self, n: int, J: int, uv: torch.Tensor, w: torch.Tensor | None = None, dtype: int = C64,
+                 oversample: int = 2, kernel_mode: int = ANALYTIC, table_samples_per_unit: int = 0,
+                 chunk: int = 0, time_stages: bool = False):
+        self._L = load_library()
+        self._h = C.c_void_p()
+        self.n, self.K, self.J, self.dtype = int(n), 2 * int(n), int(J), int(dtype)
+        opts = PurifyOpts(int(kernel_mode), int(table_samples_per_unit), int(chunk), int(bool(time_stages)))
+        M = 0 if uv is None else int(uv.shape[0])
+        self.M = M
+        rdt = _RDT.get(self.dtype, torch.float32)
+        if uv is not None:
+            if uv.dtype != rdt or uv.dim() != 2 or uv.shape[1] != 2 or not uv.is_contiguous():
+                raise ValueError(f"uv must be a contiguous [M,2] {rdt} tensor")
+        if w is not None:
+            if w.dtype != rdt or w.shape != (M,) or not w.is_contiguous():
+                raise ValueError(f"w must be a contiguous [M] {rdt} tensor")
+        on_host = uv is not None and not uv.is_cuda
+        if w is not None and uv is not None and w.is_cuda != uv.is_cuda:
+            raise ValueError("uv and w must live on the same side (both host or both device)")
+        fn = self._L.purify_op_create_host if on_host else self._L.purify_op_create
+        st = fn(C.byref(self._h), int(n), int(oversample), int(J), M,
+                C.c_void_p(uv.data_ptr()) if uv is not None and M > 0 else None,
+                C.c_void_p(w.data_ptr()) if w is not None and M > 0 else None,
+                int(dtype), C.byref(opts), _stream())
+        _check(st, "purify_op_create")
+
+    # -- lifetime
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self._L.purify_op_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    # -- facts
+    def info(self) -> dict:
+        inf = PurifyInfo()
+        _check(self._L.purify_op_info(self._h, C.byref(inf)), "purify_op_info")
+        return {k: getattr(inf, k) for k, _ in PurifyInfo._fields_}
+
+    def permutation(self) -> torch.Tensor:
+        """native -> caller index, as an int64 tensor on the device (copy)."""
+        p = C.c_void_p()
+        _check(self._L.purify_op_permutation(self._h, C.byref(p)), "purify_op_permutation")
+        if self.M == 0:
+            return torch.empty(0, dtype=torch.int64, device="cuda")
+        view = torch.as_tensor(_DeviceArray(p.value, self.M, "<i4"), device="cuda")   # zero-copy view
+        return view.to(torch.int64) & 0xFFFFFFFF
+
+    def stage_times_ms(self) -> dict:
+        arr = (C.c_float * 8)()
+        _check(self._L.purify_stage_times_ms(self._h, arr), "purify_stage_times_ms")
+        return {STAGES[i]: float(arr[i]) for i in range(7)}
+
+    def last_launch_count(self) -> int:
+        return int(self._L.purify_last_launch_count(self._h))
+
+    # -- helpers
+    def _x(self, x, name="x"):
+        if x.dtype != _CDT[self.dtype] or x.numel() != self.n * self.n or not x.is_contiguous():
+            raise ValueError(f"{name} must be a contiguous {self.n}x{self.n} {_CDT[self.dtype]} tensor")
+        return C.c_void_p(x.data_ptr())
+
+    def _y(self, y, name="y"):
+        if y.dtype != _CDT[self.dtype] or y.numel() != self.M or not y.is_contiguous():
+            raise ValueError(f"{name} must be a contiguous [{self.M}] {_CDT[self.dtype]} tensor")
+        return C.c_void_p(y.data_ptr()) if self.M > 0 else None
+
+    def _new_x(self, device="cuda"):
+        return torch.empty((self.n, self.n), dtype=_CDT[self.dtype], device=device)
+
+    def _new_y(self, device="cuda"):
+        return torch.empty(self.M, dtype=_CDT[self.dtype], device=device)
+
+    @staticmethod
+    def _dev(*ts):
+        for t in ts:
+            if not t.is_cuda:
+                raise ValueError("device entry point called with a host tensor (use the *_host methods)")
+
+    # -- Phi, Phi^dagger, Phi^dagger Phi (device buffers)
+    def degrid(self, x, y=None, native=False):
+        y = self._new_y() if y is None else y
+        self._dev(x, y)
+        fn = self._L.purify_degrid_native if native else self._L.purify_degrid
+        _check(fn(self._h, self._x(x), self._y(y), _stream()), "purify_degrid")
+        return y
+
+    def grid(self, y, x=None, native=False):
+        x = self._new_x() if x is None else x
+        self._dev(x, y)
+        fn = self._L.purify_grid_native if native else self._L.purify_grid
+        _check(fn(self._h, self._y(y), self._x(x), _stream()), "purify_grid")
+        return x
+
+    def normal(self, x, out=None):
+        out = self._new_x() if out is None else out
+        self._dev(x, out)
+        _check(self._L.purify_normal(self._h, self._x(x), self._x(out, "out"), _stream()), "purify_normal")
+        return out
+
+    def permute_to_native(self, y, out=None):
+        out = self._new_y() if out is None else out
+        self._dev(y, out)
+        _check(self._L.purify_permute_to_native(self._h, self._y(y), self._y(out), _stream()), "permute_to_native")
+        return out
+
+    def permute_from_native(self, y, out=None):
+        out = self._new_y() if out is None else out
+        self._dev(y, out)
+        _check(self._L.purify_permute_from_native(self._h, self._y(y), self._y(out), _stream()), "permute_from_native")
+        return out
+
+    # -- host-buffer (end-to-end) entry points
+    def degrid_host(self, x, y=None):
+        y = self._new_y("cpu").pin_memory() if y is None else y
+        _check(self._L.purify_degrid_host(self._h, self._x(x), self._y(y), _stream()), "purify_degrid_host")
+        return y
+
+    def grid_host(self, y, x=None):
+        x = self._new_x("cpu").pin_memory() if x is None else x
+        _check(self._L.purify_grid_host(self._h, self._y(y), self._x(x), _stream()), "purify_grid_host")
+        return x
+
+    def normal_host(self, x, out=None):
+        out = self._new_x("cpu").pin_memory() if out is None else out
+        _check(self._L.purify_normal_host(self._h, self._x(x), self._x(out, "out"), _stream()), "purify_normal_host")
+        return out
+
+    # -- single stages in the mathematical layout (tests)
+    def stage_fourier_grid(self, x):
+        B = torch.empty((self.K, self.K), dtype=_CDT[self.dtype], device="cuda")
+        _check(self._L.purify_stage_fourier_grid(self._h, self._x(x), C.c_void_p(B.data_ptr()), _stream()),
+               "purify_stage_fourier_grid")
+        return B
+
+    def stage_gridded(self, y):
+        B = torch.empty((self.K, self.K), dtype=_CDT[self.dtype], device="cuda")
+        _check(self._L.purify_stage_gridded(self._h, self._y(y), C.c_void_p(B.data_ptr()), _stream()),
+               "purify_stage_gridded")
+        return B
+
+
+class _DeviceArray:
+    """__cuda_array_interface__ wrapper of a library-owned device pointer."""
+
+    def __init__(self, ptr: int, count: int, typestr: str):
+        self.__cuda_array_interface__ = {"shape": (count,), "typestr": typestr, "data": (ptr, True), "version": 2}

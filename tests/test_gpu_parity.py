@@ -1,0 +1,255 @@
+"""Parity of the CUDA path (through the C ABI, via the ctypes binding) against the CPU oracle,
+element by element on the same seeded inputs.  -m gpu
+
+Tolerances (BASELINE.json north_star): rel-L2 <= 1e-12 for complex128, <= 1e-5 for complex64,
+over the whole output vector / image."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_1903_04502_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"c128": 1e-12, "c64": 1e-5}
+
+
+def rel_l2(a, b):
+    a = np.asarray(a, dtype=np.complex128).ravel()
+    b = np.asarray(b, dtype=np.complex128).ravel()
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def make_op(n, J, uv, w, dtype, **kw):
+    from paper_1903_04502_b200 import C64, C128, PurifyOp
+    dt = C64 if dtype == "c64" else C128
+    uvt = torch.from_numpy(np.ascontiguousarray(uv)).cuda()
+    wt = None if w is None else torch.from_numpy(np.ascontiguousarray(w)).cuda()
+    return PurifyOp(n, J, uvt, wt, dtype=dt, **kw)
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def host(t):
+    return t.detach().cpu().numpy()
+
+
+def idx_prec(dtype):
+    return 32 if dtype == "c64" else 64
+
+
+def cast_problem(x, uv, w, dtype):
+    """Round the problem to the storage precision of `dtype` (the oracle then promotes exactly)."""
+    cd, rd = synth.complex_dtype(dtype), synth.real_dtype(dtype)
+    return x.astype(cd), uv.astype(rd), None if w is None else w.astype(rd)
+
+
+def run_all_checks(x, uv, w, J, dtype, mode="analytic", R=4096, **kw):
+    """degrid (caller + native order), grid (both orders), normal, stages - all against the oracle."""
+    from paper_1903_04502_b200 import ANALYTIC, TABLE
+    n = x.shape[0]
+    tol = TOL[dtype]
+    x, uv, w = cast_problem(x, uv, w, dtype)
+    M = len(uv)
+    op = make_op(n, J, uv, w, dtype, kernel_mode=TABLE if mode == "table" else ANALYTIC,
+                 table_samples_per_unit=R if mode == "table" else 0, **kw)
+    okw = dict(mode=mode, R=R, idx_prec=idx_prec(dtype))
+    # ---- Phi
+    y_ref = oracle.degrid(x, uv, w, J, **okw)
+    y = host(op.degrid(dev(x)))
+    assert rel_l2(y, y_ref) <= tol
+    perm = host(op.permutation())
+    assert sorted(perm.tolist()) == list(range(M))
+    y_nat = host(op.degrid(dev(x), native=True))
+    assert rel_l2(y_nat, y_ref[perm]) <= tol
+    assert np.array_equal(y_nat, y[perm])                   # same numbers, different order
+    # stage: Fourier grid in the mathematical layout
+    B_ref = oracle.fft2(oracle.pad(x, J), -1)
+    assert rel_l2(host(op.stage_fourier_grid(dev(x))), B_ref) <= tol
+    # ---- Phi^dagger on random data (caller order and native order)
+    yv = synth.random_complex((M,), seed=77, dtype=dtype)
+    img_ref = oracle.grid(yv, uv, w, n, J, **okw)
+    img = host(op.grid(dev(yv)))
+    assert rel_l2(img, img_ref) <= tol
+    img_nat = host(op.grid(dev(yv[perm]), native=True))
+    assert rel_l2(img_nat, img_ref) <= tol
+    Bp_ref = oracle.grid_to_grid(yv, uv, w, 2 * n, J, **okw)
+    assert rel_l2(host(op.stage_gridded(dev(yv))), Bp_ref) <= tol
+    # permutation helpers
+    assert np.array_equal(host(op.permute_to_native(dev(yv))), yv[perm])
+    assert np.array_equal(host(op.permute_from_native(dev(yv[perm]))), yv)
+    # ---- Phi^dagger Phi
+    nrm_ref = oracle.grid(y_ref, uv, w, n, J, **okw)
+    xin = dev(x)
+    nrm = host(op.normal(xin))
+    assert rel_l2(nrm, nrm_ref) <= 2 * tol
+    # in place
+    op.normal(xin, out=xin)
+    assert rel_l2(host(xin), nrm_ref) <= 2 * tol
+    # ---- adjoint identity evaluated with GPU results
+    xr = synth.random_complex((n, n), seed=78, dtype=dtype)
+    Px = host(op.degrid(dev(xr))).astype(np.complex128)
+    Pty = img.astype(np.complex128)
+    lhs, rhs = np.vdot(Px, yv.astype(np.complex128)), np.vdot(xr.astype(np.complex128), Pty)
+    assert abs(lhs - rhs) / (np.linalg.norm(Px) * np.linalg.norm(yv)) <= 10 * tol
+    # ---- host-buffer entry points give the same numbers
+    yh = op.degrid_host(torch.from_numpy(x).pin_memory()).numpy()
+    assert np.array_equal(yh, y)
+    nh = op.normal_host(torch.from_numpy(x).pin_memory()).numpy()
+    assert rel_l2(nh, nrm_ref) <= 2 * tol
+    gh = op.grid_host(torch.from_numpy(yv).pin_memory()).numpy()
+    assert rel_l2(gh, img_ref) <= tol
+    info = op.info()
+    op.close()
+    return info
+
+
+# ------------------------------------------------------------------ config 1 (tiny)
+@pytest.mark.parametrize("J", [4, 6, 8])
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+def test_config1_tiny(J, dtype):
+    cfg, x, uv, w = synth.make_problem(1, J=J)
+    info = run_all_checks(x, uv, w, J, dtype)
+    assert info["M"] == cfg.M and info["K"] == 256
+    assert info["poly_max_abs_err"] < (2e-7 if dtype == "c64" else 2e-15)
+
+
+def test_config1_small_chunks():
+    """Many work items per tile (chunk 32/64) exercise the chunk flush / ragged tails."""
+    cfg, x, uv, w = synth.make_problem(1)
+    w = synth.rng_for(1, 1).uniform(0.5, 1.5, size=len(uv))
+    for chunk in (32, 96):
+        info = run_all_checks(x, uv, w, 4, "c128", chunk=chunk)
+        assert info["n_items"] > info["n_tiles_nonempty"]
+
+
+# ------------------------------------------------------------------ config 2
+@pytest.mark.parametrize("J", [4, 8])
+def test_config2(J):
+    cfg, x, uv, w = synth.make_problem(2, J=J)
+    info = run_all_checks(x, uv, w, J, "c128")
+    assert info["M"] == 250_000
+
+
+def test_config2_noisy_data_adjoint():
+    """BASELINE.json configs[1]: y = Phi x + noise at 30 dB; Phi^dagger y against the oracle."""
+    cfg, x, uv, w = synth.make_problem(2)
+    y0 = oracle.degrid(x, uv, w, 4)
+    y = synth.add_noise(y0, 30.0, cfg.seed)
+    assert np.linalg.norm(y - y0) / np.linalg.norm(y0) == pytest.approx(10 ** (-30 / 20), rel=0.02)
+    op = make_op(cfg.n, 4, uv, w, "c128")
+    assert rel_l2(host(op.grid(dev(y))), oracle.grid(y, uv, w, cfg.n, 4)) <= TOL["c128"]
+    op.close()
+
+
+# ------------------------------------------------------------------ table mode
+@pytest.mark.parametrize("dtype,J,R", [("c64", 4, 4096), ("c128", 4, 4096), ("c64", 6, 1000), ("c128", 8, 200000)])
+def test_table_mode(dtype, J, R):
+    cfg, x, uv, w = synth.make_problem(2, M=40_000, J=J)
+    run_all_checks(x, uv, w, J, dtype, mode="table", R=R)
+
+
+# ------------------------------------------------------------------ edge cases
+def test_wrap_and_out_of_period_uv():
+    """R8: taps that fall off the grid edge wrap; uv outside (-K/2, K/2) is taken mod K."""
+    n, K = 64, 128
+    x = synth.random_complex((n, n), seed=5)
+    rng = synth.rng_for(5, 1)
+    uv = rng.uniform(-K / 2, K / 2, size=(5000, 2))
+    uv[:6] = [(-K / 2, -K / 2), (K / 2 - 1e-9, K / 2 - 1e-9), (K / 2 - 1e-9, 0.25), (-K / 2 + 0.5, K / 2 - 0.5),
+              (K / 2 + 3.25, -K / 2 - 7.5), (5 * K + 1.5, -3 * K - 2.25)]
+    w = rng.uniform(0.5, 1.5, size=5000)
+    for dtype in ("c128", "c64"):
+        for J in (4, 8):
+            run_all_checks(x, uv, w, J, dtype)
+
+
+def test_integer_and_half_integer_uv_tie_break():
+    """R7: taps are the integers in (u - J/2, u + J/2]; crafted integer / half-integer coordinates."""
+    n = 32
+    x = synth.random_complex((n, n), seed=6)
+    g = np.arange(-20, 20)
+    uu, vv = np.meshgrid(g * 0.5, g * 0.5)
+    uv = np.stack([uu.ravel(), vv.ravel()], axis=1)
+    for dtype in ("c128", "c64"):
+        run_all_checks(x, uv, None, 4, dtype)
+        run_all_checks(x, uv, None, 6, dtype, mode="table", R=4096)
+
+
+@pytest.mark.parametrize("n", [48, 50, 22])
+def test_non_power_of_two_grid(n):
+    """K = 96 (multiple of the tile), K = 100 and K = 44 (ragged edge tiles, non-power-of-two wrap)."""
+    K = 2 * n
+    x = synth.random_complex((n, n), seed=n)
+    rng = synth.rng_for(n, 2)
+    uv = rng.uniform(-K / 2, K / 2, size=(3000, 2))
+    w = rng.uniform(0.5, 1.5, size=3000)
+    run_all_checks(x, uv, w, 4, "c128")
+    run_all_checks(x, uv, w, 6, "c64")
+
+
+def test_empty_and_single_visibility():
+    from paper_1903_04502_b200 import C128, PurifyOp
+    n = 32
+    x = synth.random_complex((n, n), seed=8)
+    op = PurifyOp(n, 4, torch.empty((0, 2), dtype=torch.float64, device="cuda"), None, dtype=C128)
+    y = op.degrid(dev(x))
+    assert y.numel() == 0
+    img = op.grid(y)
+    assert float(img.abs().max()) == 0.0
+    assert float(op.normal(dev(x)).abs().max()) == 0.0
+    op.close()
+    uv = np.array([[3.3, -7.7]])
+    run_all_checks(x, uv, np.array([1.25]), 4, "c128")
+
+
+def test_all_visibilities_in_one_cell():
+    """Degenerate distribution: one cell holds every visibility (longest possible runs)."""
+    n = 64
+    x = synth.random_complex((n, n), seed=9)
+    rng = synth.rng_for(9, 1)
+    uv = np.stack([10 + rng.uniform(0, 1, 5000), -3 + rng.uniform(0, 1, 5000)], axis=1)
+    run_all_checks(x, uv, rng.uniform(0.5, 1.5, 5000), 6, "c128", chunk=512)
+    run_all_checks(x, uv, rng.uniform(0.5, 1.5, 5000), 4, "c64")
+
+
+def test_errors():
+    from paper_1903_04502_b200 import C64, C128, PurifyError, PurifyOp
+    uv = torch.zeros((10, 2), dtype=torch.float64, device="cuda")
+    for kw, code in [(dict(n=31, J=4), -1), (dict(n=32, J=5), -1), (dict(n=32, J=4, oversample=3), -2),
+                     (dict(n=32, J=4, kernel_mode=7), -2), (dict(n=0, J=4), -1)]:
+        with pytest.raises(PurifyError) as ei:
+            PurifyOp(kw.pop("n"), kw.pop("J"), uv, None, dtype=C128, **kw)
+        assert ei.value.status == code
+    bad = uv.clone()
+    bad[3, 1] = float("nan")
+    with pytest.raises(PurifyError) as ei:
+        PurifyOp(32, 4, bad, None, dtype=C128)
+    assert ei.value.status == -3
+    bad[3, 1] = float("inf")
+    with pytest.raises(PurifyError) as ei:
+        PurifyOp(32, 4, bad, None, dtype=C128)
+    assert ei.value.status == -3
+    with pytest.raises(ValueError):
+        PurifyOp(32, 4, uv, None, dtype=C64)                 # wrong real dtype
+    op = PurifyOp(32, 4, uv, None, dtype=C128)
+    with pytest.raises(ValueError):
+        op.degrid(torch.zeros((16, 16), dtype=torch.complex128, device="cuda"))
+    op.close()
+
+
+def test_degrid_bit_reproducible_and_host_create():
+    from paper_1903_04502_b200 import C64, PurifyOp
+    cfg, x, uv, w = synth.make_problem(2, M=50_000)
+    x, uv, w = cast_problem(x, uv, w, "c64")
+    op = make_op(cfg.n, 4, uv, w, "c64")
+    a = host(op.degrid(dev(x)))
+    b = host(op.degrid(dev(x)))
+    assert np.array_equal(a, b)
+    op2 = PurifyOp(cfg.n, 4, torch.from_numpy(uv), torch.from_numpy(w), dtype=C64)   # host uv / w
+    assert np.array_equal(host(op2.degrid(dev(x))), a)
+    op.close()
+    op2.close()
