@@ -29,7 +29,11 @@ degrid_kernel(const __grid_constant__ CUtensorMap tmap, const OpParams<R> p, typ
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + sizeof(C) * BOX * BOX);
 
     const Item it = p.items[blockIdx.x];
-    const int bx0 = it.x0 - J / 2 + 1, by0 = it.y0 - J / 2 + 1;       // box origin (internal layout)
+    // box origin (internal layout).  The first column is shifted left by XOFF so that it is EVEN:
+    // a complex64 box must start on a 16-byte boundary for the TMA engine (an odd start column
+    // faults with "illegal instruction" on sm_100a).
+    constexpr int XOFF = (J / 2 - 1) & 1;
+    const int bx0 = it.x0 - J / 2 + 1 - XOFF, by0 = it.y0 - J / 2 + 1;
     const bool interior = bx0 >= 0 && by0 >= 0 && bx0 + BOX <= p.K && by0 + BOX <= p.K;
 
     if (interior) {
@@ -70,7 +74,7 @@ degrid_kernel(const __grid_constant__ CUtensorMap tmap, const OpParams<R> p, typ
         kb_weights<R, J, DEG, MODE>(uvk.y, fv, cy, p, gy);
         const int lx = wrap_idx(cx + p.Kh, p.K, p.kmask) - it.x0;
         const int ly = wrap_idx(cy + p.Kh, p.K, p.kmask) - it.y0;
-        const C* row = tile + ly * BOX + lx;
+        const C* row = tile + ly * BOX + lx + XOFF;
         R yr = (R)0, yi = (R)0;
 #pragma unroll
         for (int a = 0; a < J; ++a) {

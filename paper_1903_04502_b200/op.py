@@ -255,4 +255,4 @@ class _DeviceArray:
     """__cuda_array_interface__ wrapper of a library-owned device pointer."""
 
     def __init__(self, ptr: int, count: int, typestr: str):
-        self.__cuda_array_interface__ = {"shape": (count,), "typestr": typestr, "data": (ptr, True), "version": 2}
+        self.__cuda_array_interface__ = {"shape": (count,), "typestr": typestr, "data": (ptr, False), "version": 2}
