@@ -84,10 +84,11 @@ typedef struct {
 enum { PURIFY_STAGE_PAD = 0,   /* S + Z fused */
        PURIFY_STAGE_FFT = 1,   /* F, cuFFT                         (a2)                */
        PURIFY_STAGE_DEGRID = 2,/* W G                              (a3)                */
-       PURIFY_STAGE_GRID = 3,  /* G^dagger W^dagger incl. zeroing  (a4)                */
+       PURIFY_STAGE_GRID = 3,  /* G^dagger W^dagger kernel         (a4)                */
        PURIFY_STAGE_IFFT = 4,  /* F^dagger, cuFFT                  (a5)                */
        PURIFY_STAGE_CROP = 5,  /* Z^dagger S^dagger fused          (a6)                */
        PURIFY_STAGE_PERMUTE = 6,
+       PURIFY_STAGE_ZERO = 7,  /* zeroing of the grid before a4 (cudaMemsetAsync)      */
        PURIFY_STAGE_COUNT = 8 };
 
 /* a0: build an operator for an n x n image, K = oversample*n, J-tap Kaiser-Bessel

@@ -158,7 +158,6 @@ template <typename R, int J, int DEG> int launch_degrid_t(purify_op* op, void* y
 
 template <typename R, int J, int DEG> int launch_grid_t(purify_op* op, const void* y, bool caller_order, cudaStream_t st) {
     typedef typename pk::Cplx<R>::type C;
-    CK(cudaMemsetAsync(op->grid, 0, sizeof(C) * (size_t)op->K * op->K, st));
     if (op->n_items == 0) return PURIFY_OK;
     const size_t smem = pk::grid_smem_bytes<R, J>();
     pk::OpParams<R> p = make_params<R>(op, caller_order);
@@ -193,6 +192,10 @@ int launch_degrid(purify_op* op, void* y, bool caller_order, cudaStream_t st) {
 }
 
 int launch_grid(purify_op* op, const void* y, bool caller_order, cudaStream_t st) {
+    {
+        StageTimer tz(op, PURIFY_STAGE_ZERO, st);
+        CK(cudaMemsetAsync(op->grid, 0, csize(op) * (size_t)op->K * op->K, st));
+    }
     StageTimer t(op, PURIFY_STAGE_GRID, st);
     if (op->dtype == PURIFY_C64) {
         switch (op->J) {

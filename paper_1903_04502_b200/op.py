@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libpurify_op.so")
 
 C64, C128 = 0, 1
 ANALYTIC, TABLE = 0, 1
-STAGES = ("pad", "fft", "degrid", "grid", "ifft", "crop", "permute", "reserved")
+STAGES = ("pad", "fft", "degrid", "grid", "ifft", "crop", "permute", "zero")
 
 # every symbol include/purify_op.h declares (checked by tests/test_abi.py)
 SYMBOLS = (
@@ -160,7 +160,7 @@ class PurifyOp:
     def stage_times_ms(self) -> dict:
         arr = (C.c_float * 8)()
         _check(self._L.purify_stage_times_ms(self._h, arr), "purify_stage_times_ms")
-        return {STAGES[i]: float(arr[i]) for i in range(7)}
+        return {STAGES[i]: float(arr[i]) for i in range(8)}
 
     def last_launch_count(self) -> int:
         return int(self._L.purify_last_launch_count(self._h))
