@@ -18,8 +18,10 @@
  *           (paper's radians/pixel omega: u = omega K / 2 pi).  Any finite value with
  *           |u| < 2^30 is accepted and taken mod K.
  *   dtype   PURIFY_C64 : x, y complex64,  uv and w float32.   PURIFY_C128: complex128 / float64.
- *   order   "caller order" = the order of uv at create.  "native order" = the library's tile-sorted
- *           order; native[i] = caller[perm[i]] with perm from purify_op_permutation().
+ *   order   "caller order" = the order of uv at create.  "native order" = the library's own order, a
+ *           vector of M_native >= M entries (purify_op_info): native[i] = caller[perm[i]] with perm
+ *           from purify_op_permutation(); perm[i] = 0xFFFFFFFF marks a PADDING entry (complex64
+ *           layout only): purify_degrid_native writes 0 there, purify_grid_native ignores it.
  *   memory  "_dev" pointers are CUDA device pointers on the current device, "_host" pointers are
  *           host pointers (pinned memory recommended).  The caller owns every buffer it passes; the
  *           handle owns its sorted copies, tables, grid workspace and cuFFT plan.
@@ -77,7 +79,11 @@ typedef struct {
     int poly_degree;            /* ANALYTIC: degree of the per-tap polynomial in the cell offset     */
     double poly_max_abs_err;    /* ANALYTIC: max |poly - g| over the support (fit check at create)   */
     long long device_bytes;     /* device memory owned by the handle                                 */
-    long long max_tile_count;   /* visibilities in the fullest tile                                  */
+    long long max_tile_count;   /* visibilities in the fullest tile / band                           */
+    long long M_native;         /* length of a native-order y vector (>= M: the complex64 layout pads) */
+    long long n_batches;        /* complex64 layout: batches of 32 cell-units                        */
+    int layout;                 /* 0 = tile-sorted (complex128), 1 = batched cell-stationary (complex64) */
+    int tile_h;                 /* tile / band height in grid cells (tile = width)                   */
 } purify_info;
 
 /* Stage indices for purify_stage_times_ms (milliseconds of the LAST call that ran the stage). */
@@ -105,7 +111,8 @@ int purify_op_create_host(purify_op **out, int n, int oversample, int J, long lo
                           const purify_opts *opts, void *cuda_stream);
 int purify_op_destroy(purify_op *op);
 int purify_op_info(const purify_op *op, purify_info *info);
-/* perm_dev[i] = caller index of the visibility at native position i (device pointer, M entries). */
+/* perm_dev[i] = caller index of the visibility at native position i, or 0xFFFFFFFF for padding
+ * (device pointer, M_native entries). */
 int purify_op_permutation(const purify_op *op, const unsigned **perm_dev);
 
 /* Phi (a1-a3):  x_dev[n*n] -> y_dev[M], caller order. */

@@ -1,0 +1,540 @@
+// complex64 hot path: the "cell-stationary" batched layout and its create-time construction (a0).
+//
+// Why (profiles/r1a_summary.md): with one thread per visibility both W G and its adjoint are bound
+// by the fp32 pipe / issue rate, not by HBM (235 lane-instructions per visibility at J = 6), and the
+// adjoint additionally pays shared-memory read-modify-writes per visibility.  Here a THREAD OWNS A
+// GRID CELL for a run of visibilities: degridding keeps the cell's J x J patch of the Fourier grid
+// in registers, gridding keeps the J x J accumulators in registers, and the inner loop over the
+// run's visibilities touches no shared memory at all.  The 2J^2 complex x real MACs and the paired
+// Horner chains of the kernel weights are issued as packed fp32 (FFMA2, fma.rn.f32x2, sm_100).
+//
+// Layout (built once at create):
+//   band   32 x 16 cells of the oversampled grid (internal DC-centred layout); one WARP works on one
+//          band at a time with a private (16+J-1) x (32+J) shared-memory box.
+//   unit   up to UNIT_CAP visibilities of ONE cell (a cell with more is split into several units).
+//   batch  32 units, one per lane, processed in lockstep for n_iter = max count iterations.  The 16
+//          lanes of a half-warp hold cells of 16 different residues (ly*BOXW + lx) mod 16, so the
+//          8-byte shared-memory accesses of a half-warp hit 16 different bank pairs (conflict-free);
+//          the units of a residue class are handed out in descending count order, so the counts in a
+//          batch are nearly equal (lane efficiency 0.8-0.9 for Poisson-like cell counts).
+//   slots  visibility data in "native order": slot = 32*(base32 + i) + lane for iteration i of a
+//          batch - coalesced.  Slots past a unit's count are padding: perm = 0xFFFFFFFF, w = 0,
+//          uv = the cell centre, y_native = 0.
+//   item   a run of batches of one band with at most ITEM_ITERS iterations: the unit of dynamic
+//          scheduling (persistent warps pull items from an atomic counter).
+#pragma once
+#include "kernels.cuh"
+
+namespace pk {
+
+constexpr int XBW = 32, XBH = 16, XCELLS = XBW * XBH;   // band geometry
+constexpr int UNIT_CAP = 64;                            // visibilities per unit (L)
+constexpr int ITEM_ITERS = 256;                         // iterations per item
+constexpr unsigned PERM_PAD = 0xFFFFFFFFu;
+
+template <int J> struct XCfg {
+    static constexpr int XOFF = (J / 2 - 1) & 1;        // makes the box's first column even (TMA: 16-byte aligned)
+    static constexpr int BOXW = XBW + J;                // columns (even)
+    static constexpr int BOXH = XBH + J - 1;            // rows
+    static constexpr int REGION_BYTES = ((BOXW * BOXH * 8 + 127) / 128) * 128;
+    static constexpr int WARPS = 4;
+    static constexpr int THREADS = WARPS * 32;
+};
+
+struct XItem {
+    int x0, y0;          // band origin, internal layout
+    int begin, end;      // batch range
+};
+
+struct XParams {
+    float2* grid;                 // K*K, internal layout
+    int K, Kh, kmask;
+    const XItem* items;
+    int n_items;
+    unsigned* counter;            // dynamic item queue (reset before every launch)
+    const uint2* bhdr;            // per batch: x = base32, y = n_iter | flags << 16 (bit 0: duplicate cell => 2-pass flush)
+    const unsigned* blane;        // per batch 32 lane words: cell (ly << 5 | lx) | count << 16
+    const float2* uv;             // slots
+    const float* w;               // slots
+    const unsigned* perm;         // slots -> caller index (PERM_PAD for padding); nullptr = native-order y
+    KbCoef<float> coef;
+    const float* table;
+    float table_R;
+    int table_len;
+};
+
+// class (residue) of cell (ly, lx) for box pitch boxw, and the inverse enumeration of a class' 32 members
+__host__ __device__ __forceinline__ int x_class(int ly, int lx, int boxw) { return (ly * boxw + lx) & 15; }
+__host__ __device__ __forceinline__ int x_member_cell(int r, int m, int boxw) {
+    const int ly = m >> 1;
+    const int lx = ((r - ly * boxw) & 15) + 16 * (m & 1);
+    return ly * XBW + lx;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a0.1: reduce (u, v) to the principal period, key = band * 512 + cell (band-major).
+__global__ void xkey_kernel(const float2* __restrict__ uv, long long M, int K, int nbx,
+                            unsigned* __restrict__ keys, unsigned* __restrict__ idx, int* __restrict__ bad) {
+    for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < M; k += (long long)gridDim.x * blockDim.x) {
+        const float2 c = uv[k];
+        unsigned key = 0;
+        if (!(fabsf(c.x) < 1073741824.0f) || !(fabsf(c.y) < 1073741824.0f)) {
+            atomicOr(bad, 1);
+        } else {
+            const long long fx = (long long)floorf(c.x) + K / 2, fy = (long long)floorf(c.y) + K / 2;
+            long long gx = fx % K, gy = fy % K;
+            if (gx < 0) gx += K;
+            if (gy < 0) gy += K;
+            const unsigned band = (unsigned)(gy / XBH) * nbx + (unsigned)(gx / XBW);
+            key = band * XCELLS + (unsigned)(gy % XBH) * XBW + (unsigned)(gx % XBW);
+        }
+        keys[k] = key;
+        idx[k] = (unsigned)k;
+    }
+}
+
+// principal-period coordinate: u - m K with m = floor((floor(u) + K/2) / K); exact (double arithmetic,
+// the result is a multiple of ulp(u) of small magnitude, hence a float).
+__device__ __forceinline__ float x_reduce(float u, int K) {
+    const long long f = (long long)floorf(u) + K / 2;
+    long long m = f / K;
+    if (f % K < 0) --m;
+    return (float)((double)u - (double)m * (double)K);
+}
+
+__global__ void band_start_kernel(const unsigned* __restrict__ keys, long long M, int n_bands, unsigned* __restrict__ band_start) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t > n_bands) return;
+    const unsigned long long target = (unsigned long long)t * XCELLS;
+    long long lo = 0, hi = M;
+    while (lo < hi) {
+        const long long mid = (lo + hi) >> 1;
+        if ((unsigned long long)keys[mid] < target) lo = mid + 1; else hi = mid;
+    }
+    band_start[t] = (unsigned)lo;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a0.2 / a0.3: per-band batch construction.  One CTA of 512 threads per band; thread t <-> (class
+// r = t >> 5, member m = t & 31).  PASS 1 counts batches / iterations / items, PASS 2 (after the
+// exclusive scans over bands) writes batch headers, lane words, unit sources and items.
+struct BandTotals { unsigned nb, iters, items; };
+
+template <int PASS>
+__global__ void __launch_bounds__(XCELLS)
+band_build_kernel(const unsigned* __restrict__ keys, const unsigned* __restrict__ band_start, int nbx, int boxw,
+                  BandTotals* __restrict__ totals,                      // PASS 1 out
+                  const unsigned* __restrict__ nb_off, const unsigned* __restrict__ iter_off,
+                  const unsigned* __restrict__ item_off,                // PASS 2 in (exclusive scans)
+                  uint2* __restrict__ bhdr, unsigned* __restrict__ blane, unsigned* __restrict__ lsrc,
+                  XItem* __restrict__ items) {
+    __shared__ unsigned s_full[16][32], s_rem[16][32], s_start[16][32];
+    __shared__ unsigned s_F[16], s_R[16], s_maxfull[16];
+    __shared__ unsigned s_remsorted[16][32];
+    __shared__ unsigned s_scan[XCELLS];
+    __shared__ unsigned s_ni[XCELLS];
+    __shared__ unsigned s_carry, s_lastni, s_Q;
+
+    const int band = blockIdx.x;
+    const unsigned bs = band_start[band], be = band_start[band + 1];
+    const int t = threadIdx.x, r = t >> 5, m = t & 31;
+    if (bs == be) {
+        if (PASS == 1 && t == 0) { totals[band].nb = 0; totals[band].iters = 0; totals[band].items = 0; }
+        return;
+    }
+    // --- cell counts
+    const int cell = x_member_cell(r, m, boxw);
+    {
+        const unsigned long long k0 = (unsigned long long)band * XCELLS + cell;
+        unsigned lo = bs, hi = be;
+        while (lo < hi) { const unsigned mid = lo + ((hi - lo) >> 1); if (keys[mid] < k0) lo = mid + 1; else hi = mid; }
+        unsigned lo2 = lo, hi2 = be;
+        while (lo2 < hi2) { const unsigned mid = lo2 + ((hi2 - lo2) >> 1); if (keys[mid] <= k0) lo2 = mid + 1; else hi2 = mid; }
+        const unsigned cnt = lo2 - lo;
+        s_start[r][m] = lo;
+        s_full[r][m] = cnt / UNIT_CAP;
+        s_rem[r][m] = cnt % UNIT_CAP;
+    }
+    __syncthreads();
+    // --- per-class totals and remainder ranks (descending, ties by member index)
+    const unsigned myfull = s_full[r][m], myrem = s_rem[r][m];
+    unsigned rank = 0, F = 0, R = 0, maxfull = 0;
+    for (int q = 0; q < 32; ++q) {
+        const unsigned f = s_full[r][q], e = s_rem[r][q];
+        F += f; R += (e > 0); maxfull = max(maxfull, f);
+        if (e > myrem || (e == myrem && q < m)) ++rank;
+    }
+    if (m == 0) { s_F[r] = F; s_R[r] = R; s_maxfull[r] = maxfull; }
+    s_remsorted[r][rank] = myrem;            // ranks are a permutation of 0..31 (zeros sort last)
+    __syncthreads();
+    if (t == 0) {
+        unsigned Q = 0;
+        for (int q = 0; q < 16; ++q) Q = max(Q, s_F[q] + s_R[q]);
+        s_Q = Q; s_carry = 0; s_lastni = 0;
+    }
+    __syncthreads();
+    const unsigned Q = s_Q, NB = (Q + 1) >> 1;
+
+    // count of the unit at queue position g of class q
+    auto unit_count = [&](int q, unsigned g) -> unsigned {
+        const unsigned Fq = s_F[q];
+        if (g < Fq) return UNIT_CAP;
+        const unsigned j = g - Fq;
+        return j < 32 ? s_remsorted[q][j] : 0u;
+    };
+
+    const unsigned nb0 = PASS == 2 ? nb_off[band] : 0, it0 = PASS == 2 ? iter_off[band] : 0,
+                   item0 = PASS == 2 ? item_off[band] : 0;
+    const int x0 = (band % nbx) * XBW, y0 = (band / nbx) * XBH;
+
+    // --- batches: n_iter, prefix of iterations, item boundaries (chunks of 512 batches)
+    unsigned total_iters = 0;
+    for (unsigned base = 0; base < NB; base += XCELLS) {
+        const unsigned b = base + t;
+        unsigned ni = 0;
+        if (b < NB)
+            for (int q = 0; q < 16; ++q) ni = max(ni, max(unit_count(q, 2 * b), unit_count(q, 2 * b + 1)));
+        // block-wide inclusive scan of ni
+        s_ni[t] = ni;
+        s_scan[t] = ni;
+        __syncthreads();
+        for (int off = 1; off < XCELLS; off <<= 1) {
+            const unsigned v = t >= off ? s_scan[t - off] : 0;
+            __syncthreads();
+            s_scan[t] += v;
+            __syncthreads();
+        }
+        const unsigned carry = s_carry;
+        const unsigned incl = s_scan[t] + carry, excl = incl - ni;
+        if (PASS == 2 && b < NB) {
+            bhdr[nb0 + b] = make_uint2(it0 + excl, ni);                 // flags are OR-ed in below
+            // item of a batch = floor(iterations before it / ITEM_ITERS); a batch opens an item when
+            // its predecessor belongs to another one
+            const unsigned item = excl / ITEM_ITERS;
+            const unsigned ni_prev = t > 0 ? s_ni[t - 1] : s_lastni;
+            const bool first = b == 0 || item != (excl - ni_prev) / ITEM_ITERS;
+            if (first) {
+                items[item0 + item].x0 = x0;
+                items[item0 + item].y0 = y0;
+                items[item0 + item].begin = (int)(nb0 + b);
+                if (item > 0) items[item0 + item - 1].end = (int)(nb0 + b);
+            }
+            if (b == NB - 1) items[item0 + item].end = (int)(nb0 + NB);
+        }
+        __syncthreads();
+        if (t == XCELLS - 1) { s_carry = incl; s_lastni = ni; }
+        __syncthreads();
+        total_iters = s_carry;
+    }
+    if (PASS == 1) {
+        if (t == 0) {
+            totals[band].nb = NB;
+            totals[band].iters = total_iters;
+            // items = distinct values of floor(excl(b) / ITEM_ITERS); excl of the last batch = total - n_iter(last)
+            unsigned last_ni = 0;
+            for (int q = 0; q < 16; ++q) last_ni = max(last_ni, max(unit_count(q, 2 * (NB - 1)), unit_count(q, 2 * (NB - 1) + 1)));
+            totals[band].items = (total_iters - last_ni) / ITEM_ITERS + 1;
+        }
+        return;
+    }
+    // ---------------- PASS 2: lane words (idle default first), then every thread emits its cell's units
+    for (unsigned i = t; i < NB * 32; i += XCELLS) { blane[(size_t)nb0 * 32 + i] = 0; lsrc[(size_t)nb0 * 32 + i] = 0; }
+    __syncthreads();
+    auto emit = [&](unsigned g, unsigned count, unsigned src) {
+        const unsigned b = g >> 1, lane = (g & 1) * 16 + r;
+        blane[(size_t)(nb0 + b) * 32 + lane] = (unsigned)cell | (count << 16);
+        lsrc[(size_t)(nb0 + b) * 32 + lane] = src;
+    };
+    // full units in layer-major order: unit (m, j) at  g = sum_q min(full_q, j) + #{q < m : full_q > j}
+    {
+        unsigned G = 0;                                   // sum_q min(full_q, j)
+        for (unsigned j = 0; j < myfull; ++j) {
+            unsigned Nj = 0, pos = 0, lastq = 0;
+            for (int q = 0; q < 32; ++q) {
+                const bool in = s_full[r][q] > j;
+                Nj += in; if (in && q < m) ++pos; if (in) lastq = q;
+            }
+            const unsigned g = G + pos;
+            emit(g, UNIT_CAP, s_start[r][m] + j * UNIT_CAP);
+            // duplicate-cell check: odd g whose predecessor (g - 1) is the same cell
+            if ((g & 1) && pos == 0 && j > 0) {
+                unsigned lastprev = 0;
+                for (int q = 0; q < 32; ++q) if (s_full[r][q] > j - 1) lastprev = q;
+                if (lastprev == (unsigned)m) atomicOr(&bhdr[nb0 + (g >> 1)].y, 1u << 16);
+            }
+            (void)lastq;
+            G += Nj;
+        }
+    }
+    if (myrem > 0) {
+        const unsigned g = s_F[r] + rank;
+        emit(g, myrem, s_start[r][m] + myfull * UNIT_CAP);
+        if ((g & 1) && rank == 0 && myfull > 0) {
+            unsigned lastprev = 0;
+            for (int q = 0; q < 32; ++q) if (s_full[r][q] > s_maxfull[r] - 1) lastprev = q;
+            if (lastprev == (unsigned)m && myfull == s_maxfull[r]) atomicOr(&bhdr[nb0 + (g >> 1)].y, 1u << 16);
+        }
+    }
+}
+
+__global__ void split_totals_kernel(const BandTotals* __restrict__ t, int n_bands, unsigned* __restrict__ nb,
+                                    unsigned* __restrict__ iters, unsigned* __restrict__ items, unsigned* __restrict__ nonempty) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i > n_bands) return;
+    if (i == n_bands) { nb[i] = 0; iters[i] = 0; items[i] = 0; return; }
+    nb[i] = t[i].nb; iters[i] = t[i].iters; items[i] = t[i].items;
+    if (t[i].nb) atomicAdd(nonempty, 1u);
+}
+
+// a0.4: fill the slots of every batch (one warp per batch): permutation, reduced (u, v), weights.
+__global__ void __launch_bounds__(256)
+slot_fill_kernel(const uint2* __restrict__ bhdr, const unsigned* __restrict__ blane, const unsigned* __restrict__ lsrc,
+                 unsigned n_batches, const unsigned* __restrict__ perm0, const float2* __restrict__ uv,
+                 const float* __restrict__ w, int K,
+                 unsigned* __restrict__ perm, float2* __restrict__ uv_s, float* __restrict__ w_s) {
+    const unsigned warps = (gridDim.x * blockDim.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    for (unsigned b = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; b < n_batches; b += warps) {
+        const uint2 h = bhdr[b];
+        const unsigned n_iter = h.y & 0xFFFFu;
+        const unsigned lw = blane[(size_t)b * 32 + lane], src = lsrc[(size_t)b * 32 + lane];
+        const unsigned cnt = lw >> 16;
+        float2 pad = make_float2(0.f, 0.f);
+        if (cnt > 0) {                                     // padding coordinate: the unit's first visibility
+            const float2 c = uv[perm0[src]];
+            pad = make_float2(x_reduce(c.x, K), x_reduce(c.y, K));
+        }
+        for (unsigned i = 0; i < n_iter; ++i) {
+            const size_t slot = ((size_t)h.x + i) * 32 + lane;
+            if (i < cnt) {
+                const unsigned p = perm0[src + i];
+                const float2 c = uv[p];
+                perm[slot] = p;
+                uv_s[slot] = make_float2(x_reduce(c.x, K), x_reduce(c.y, K));
+                w_s[slot] = w ? w[p] : 1.f;
+            } else {
+                perm[slot] = PERM_PAD;
+                uv_s[slot] = pad;
+                w_s[slot] = 0.f;
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// packed fp32 helpers (sm_100 FFMA2 / FMUL2 / FADD2)
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ float2 mul2(float2 a, float2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 dup2(float a) { return make_float2(a, a); }
+
+// Kernel weights of both axes of one visibility in a known cell: g[j] = (g_x[j], g_y[j]) for the taps
+// c_j = cell - J/2 + 1 + j.  ANALYTIC: t = (u - cell) - 1/2 per axis, the even / odd Horner chains of
+// the two axes run as one packed chain.  TABLE: T[floor(|u - c_j| R + 1/2)], one IEEE op per step.
+template <int J, int DEG, int MODE>
+__device__ __forceinline__ void x_weights(float2 uv, float2 cellf, int cx, int cy, const XParams& p, float2 (&g)[J]) {
+    if (MODE == 0) {
+        constexpr int NE = DEG / 2 + 1, NO = (DEG + 1) / 2;
+        const float2 t = add2(add2(uv, make_float2(-cellf.x, -cellf.y)), make_float2(-0.5f, -0.5f));
+        const float2 t2 = mul2(t, t), nt = make_float2(-t.x, -t.y);
+#pragma unroll
+        for (int j = 0; j < J / 2; ++j) {
+            float2 E = dup2(p.coef.e[j][NE - 1]), O = dup2(p.coef.o[j][NO - 1]);
+#pragma unroll
+            for (int m = NE - 2; m >= 0; --m) E = fma2(E, t2, dup2(p.coef.e[j][m]));
+#pragma unroll
+            for (int m = NO - 2; m >= 0; --m) O = fma2(O, t2, dup2(p.coef.o[j][m]));
+            g[j] = fma2(t, O, E);
+            g[J - 1 - j] = fma2(nt, O, E);
+        }
+    } else {
+#pragma unroll
+        for (int j = 0; j < J; ++j) {
+            const int ox = cx - J / 2 + 1 + j, oy = cy - J / 2 + 1 + j;
+            const float dx = __fsub_rn(uv.x, (float)ox), dy = __fsub_rn(uv.y, (float)oy);
+            const int ix = (int)floorf(__fadd_rn(__fmul_rn(fabsf(dx), p.table_R), 0.5f));
+            const int iy = (int)floorf(__fadd_rn(__fmul_rn(fabsf(dy), p.table_R), 0.5f));
+            g[j].x = ix < p.table_len ? __ldg(p.table + ix) : 0.f;
+            g[j].y = iy < p.table_len ? __ldg(p.table + iy) : 0.f;
+        }
+    }
+}
+
+__device__ __forceinline__ unsigned x_next_item(unsigned* counter, int lane) {
+    unsigned it = 0;
+    if (lane == 0) it = atomicAdd(counter, 1u);
+    return __shfl_sync(0xffffffffu, it, 0);
+}
+
+// ---------------------------------------------------------------------------------------------
+// a3 (complex64): W G.  Persistent warps; per item the band's box is staged by one TMA load into the
+// warp's private shared-memory region; per batch every lane loads its cell's J x J patch into
+// registers (conflict-free 8-byte loads) and then runs its unit's visibilities out of registers.
+// HBM per slot: uv 8 + w 4 read, y 8 written (+ perm 4 and a scattered 8-byte store in caller order).
+template <int J, int DEG, int MODE, int CALLER>
+__global__ void __launch_bounds__(XCfg<J>::THREADS)
+degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float2* __restrict__ y) {
+    typedef XCfg<J> Cfg;
+    constexpr int BOXW = Cfg::BOXW, BOXH = Cfg::BOXH, XOFF = Cfg::XOFF;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    float2* tile = reinterpret_cast<float2*>(smem_raw + warp * Cfg::REGION_BYTES);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + Cfg::WARPS * Cfg::REGION_BYTES) + warp;
+    if (lane == 0) { mbar_init(bar, 1); fence_barrier_init(); }
+    __syncwarp();
+    uint32_t phase = 0;
+
+    for (unsigned item = x_next_item(p.counter, lane); item < (unsigned)p.n_items; item = x_next_item(p.counter, lane)) {
+        const XItem it = p.items[item];
+        const int bx0 = it.x0 - (J / 2 - 1) - XOFF, by0 = it.y0 - (J / 2 - 1);
+        const bool interior = bx0 >= 0 && by0 >= 0 && bx0 + BOXW <= p.K && by0 + BOXH <= p.K;
+        __syncwarp();                                   // every lane is done with the previous box
+        if (interior) {
+            if (lane == 0) {
+                fence_proxy_async();
+                mbar_expect_tx(bar, (uint32_t)(sizeof(float2) * BOXW * BOXH));
+                tma_load_2d(tile, &tmap, 2 * bx0, by0, bar);
+            }
+            mbar_wait(bar, phase);
+            phase ^= 1;
+        } else {
+            for (int i = lane; i < BOXW * BOXH; i += 32) {
+                const int r = wrap_idx(by0 + i / BOXW, p.K, p.kmask), c = wrap_idx(bx0 + i % BOXW, p.K, p.kmask);
+                tile[i] = p.grid[(long long)r * p.K + c];
+            }
+            __syncwarp();
+        }
+        for (int b = it.begin; b < it.end; ++b) {
+            const uint2 h = p.bhdr[b];
+            const unsigned lw = p.blane[(size_t)b * 32 + lane];
+            const int n_iter = (int)(h.y & 0xFFFFu);
+            const int ly = (lw >> 5) & 15, lx = lw & 31;
+            const int cx = it.x0 + lx - p.Kh, cy = it.y0 + ly - p.Kh;       // cell = floor(u'), floor(v')
+            const float2 cellf = make_float2((float)cx, (float)cy);
+            float2 B[J][J];
+            {
+                const float2* src = tile + ly * BOXW + lx + XOFF;
+#pragma unroll
+                for (int a = 0; a < J; ++a)
+#pragma unroll
+                    for (int c = 0; c < J; ++c) B[a][c] = src[a * BOXW + c];
+            }
+            size_t slot = (size_t)h.x * 32 + lane;
+            float2 uvk = p.uv[slot];
+            float wk = p.w[slot];
+            for (int i = 0; i < n_iter; ++i) {
+                float2 uvn = uvk;
+                float wn = 0.f;
+                if (i + 1 < n_iter) { uvn = p.uv[slot + 32]; wn = p.w[slot + 32]; }
+                float2 g[J];
+                x_weights<J, DEG, MODE>(uvk, cellf, cx, cy, p, g);
+                float2 acc = make_float2(0.f, 0.f);
+#pragma unroll
+                for (int a = 0; a < J; ++a) {
+                    float2 row = mul2(dup2(g[0].x), B[a][0]);
+#pragma unroll
+                    for (int c = 1; c < J; ++c) row = fma2(dup2(g[c].x), B[a][c], row);
+                    acc = fma2(dup2(g[a].y), row, acc);
+                }
+                const float2 out = mul2(dup2(wk), acc);                     // padding slots: w = 0 -> 0
+                if (CALLER) {
+                    const unsigned pi = p.perm[slot];
+                    if (pi != PERM_PAD) y[pi] = out;
+                } else {
+                    y[slot] = out;
+                }
+                slot += 32; uvk = uvn; wk = wn;
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a4 (complex64): G^dagger W^dagger.  Same items / batches.  Every lane accumulates its unit's
+// J x J outer products in registers; at the end of the batch the accumulators are added into the
+// warp's private shared-memory box (lanes of one pass hold distinct cells => distinct addresses in
+// every step, no atomics; __syncwarp orders the steps because footprints of different lanes overlap);
+// at the end of the item the box is added to the global grid with one 8-byte reduction per non-zero
+// cell (RED.ADD.F32x2; halos of neighbouring bands and the items of one band meet there).
+template <int J, int DEG, int MODE, int CALLER>
+__global__ void __launch_bounds__(XCfg<J>::THREADS)
+grid_x_kernel(const XParams p, const float2* __restrict__ y) {
+    typedef XCfg<J> Cfg;
+    constexpr int BOXW = Cfg::BOXW, BOXH = Cfg::BOXH, XOFF = Cfg::XOFF;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    float2* tile = reinterpret_cast<float2*>(smem_raw + warp * Cfg::REGION_BYTES);
+
+    for (unsigned item = x_next_item(p.counter, lane); item < (unsigned)p.n_items; item = x_next_item(p.counter, lane)) {
+        const XItem it = p.items[item];
+        for (int i = lane; i < BOXW * BOXH; i += 32) tile[i] = make_float2(0.f, 0.f);
+        __syncwarp();
+        for (int b = it.begin; b < it.end; ++b) {
+            const uint2 h = p.bhdr[b];
+            const unsigned lw = p.blane[(size_t)b * 32 + lane];
+            const int n_iter = (int)(h.y & 0xFFFFu);
+            const bool two_pass = (h.y >> 16) & 1u;
+            const int cnt = (int)(lw >> 16);
+            const int ly = (lw >> 5) & 15, lx = lw & 31;
+            const int cx = it.x0 + lx - p.Kh, cy = it.y0 + ly - p.Kh;
+            const float2 cellf = make_float2((float)cx, (float)cy);
+            float2 A[J][J];
+#pragma unroll
+            for (int a = 0; a < J; ++a)
+#pragma unroll
+                for (int c = 0; c < J; ++c) A[a][c] = make_float2(0.f, 0.f);
+
+            size_t slot = (size_t)h.x * 32 + lane;
+            auto load_y = [&](size_t s, bool ok) -> float2 {
+                if (!ok) return make_float2(0.f, 0.f);
+                if (CALLER) return y[p.perm[s]];
+                return y[s];
+            };
+            float2 uvk = p.uv[slot];
+            float wk = p.w[slot];
+            float2 yk = load_y(slot, 0 < cnt);
+            for (int i = 0; i < n_iter; ++i) {
+                float2 uvn = uvk, yn = make_float2(0.f, 0.f);
+                float wn = 0.f;
+                if (i + 1 < n_iter) { uvn = p.uv[slot + 32]; wn = p.w[slot + 32]; yn = load_y(slot + 32, i + 1 < cnt); }
+                float2 g[J];
+                x_weights<J, DEG, MODE>(uvk, cellf, cx, cy, p, g);
+                const float2 z = mul2(dup2(wk), yk);                        // padding: w = 0 and y = 0
+#pragma unroll
+                for (int a = 0; a < J; ++a) {
+                    const float2 q = mul2(dup2(g[a].y), z);
+#pragma unroll
+                    for (int c = 0; c < J; ++c) A[a][c] = fma2(dup2(g[c].x), q, A[a][c]);
+                }
+                slot += 32; uvk = uvn; wk = wn; yk = yn;
+            }
+            // ---- flush the accumulators into the warp's box.  Idle lanes (no unit) stay out; a batch
+            // that holds one cell twice (lanes r and 16 + r) flushes its two half-warps one after the other.
+            float2* dst = tile + ly * BOXW + lx + XOFF;
+            const int n_pass = two_pass ? 2 : 1;
+            for (int pass = 0; pass < n_pass; ++pass) {
+                const bool act = cnt > 0 && (!two_pass || (lane >> 4) == pass);
+#pragma unroll
+                for (int a = 0; a < J; ++a)
+#pragma unroll
+                    for (int c = 0; c < J; ++c) {
+                        if (act) dst[a * BOXW + c] = add2(dst[a * BOXW + c], A[a][c]);
+                        __syncwarp();
+                    }
+            }
+        }
+        // ---- add the box to the global grid (periodic wrap here)
+        __syncwarp();
+        const int bx0 = it.x0 - (J / 2 - 1) - XOFF, by0 = it.y0 - (J / 2 - 1);
+        for (int i = lane; i < BOXW * BOXH; i += 32) {
+            const float2 v = tile[i];
+            if (v.x != 0.f || v.y != 0.f) {
+                const int r = wrap_idx(by0 + i / BOXW, p.K, p.kmask), c = wrap_idx(bx0 + i % BOXW, p.K, p.kmask);
+                atomicAdd(p.grid + (long long)r * p.K + c, v);
+            }
+        }
+        __syncwarp();
+    }
+}
+
+}  // namespace pk

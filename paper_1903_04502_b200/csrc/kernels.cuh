@@ -108,15 +108,15 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t phase) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_LOOP:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra WAIT_DONE;\n"
-        "bra WAIT_LOOP;\n"
-        "WAIT_DONE:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(phase) : "memory");
+    uint32_t done = 0;
+    while (!done) {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n" : "=r"(done) : "r"(smem_u32(bar)), "r"(phase) : "memory");
+    }
 }
 __device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* tmap, int x, int y, uint64_t* bar) {
     asm volatile(
@@ -270,9 +270,11 @@ __global__ void fill_items_kernel(const int* __restrict__ tile_start, const int*
 
 template <typename C>
 __global__ void permute_kernel(const C* __restrict__ in, C* __restrict__ out, const unsigned* __restrict__ perm,
-                               long long M, int to_native) {
-    for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < M; k += (long long)gridDim.x * blockDim.x) {
-        if (to_native) out[k] = in[perm[k]]; else out[perm[k]] = in[k];
+                               long long M_native, int to_native) {
+    for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < M_native; k += (long long)gridDim.x * blockDim.x) {
+        const unsigned pi = perm[k];
+        if (to_native) { C z; z.x = 0; z.y = 0; out[k] = pi == 0xFFFFFFFFu ? z : in[pi]; }
+        else if (pi != 0xFFFFFFFFu) out[pi] = in[k];
     }
 }
 

@@ -15,6 +15,7 @@
 #include <new>
 #include <vector>
 
+#include "batched.cuh"
 #include "degrid.cuh"
 #include "grid.cuh"
 #include "kb_host.hpp"
@@ -92,6 +93,17 @@ struct purify_op {
     bool ev_ok = false;
     bool stage_ran[PURIFY_STAGE_COUNT];
     int launches = 0;
+    // complex64 batched ("cell-stationary") layout, batched.cuh
+    bool batched = false;
+    long long M_native = 0;       // slots (batched) or M (sorted layout)
+    int n_bands = 0, n_bands_nonempty = 0;
+    unsigned n_batches = 0;
+    uint2* x_bhdr = nullptr;
+    unsigned* x_blane = nullptr;
+    pk::XItem* x_items = nullptr;
+    unsigned* x_counter = nullptr;
+    CUtensorMap tmap_x;
+    int x_ctas_degrid = 0, x_ctas_grid = 0;
 };
 
 namespace {
@@ -175,8 +187,101 @@ template <typename R, int J, int DEG> int launch_grid_t(purify_op* op, const voi
     return PURIFY_OK;
 }
 
+pk::XParams make_xparams(const purify_op* op, bool caller_order) {
+    pk::XParams p;
+    p.grid = (float2*)op->grid;
+    p.K = op->K; p.Kh = op->K / 2;
+    p.kmask = (op->K & (op->K - 1)) == 0 ? op->K - 1 : 0;
+    p.items = op->x_items;
+    p.n_items = op->n_items;
+    p.counter = op->x_counter;
+    p.bhdr = op->x_bhdr;
+    p.blane = op->x_blane;
+    p.uv = (const float2*)op->uv_s;
+    p.w = (const float*)op->w_s;
+    p.perm = caller_order ? op->perm : nullptr;
+    memcpy(&p.coef, &op->coef32, sizeof(p.coef));
+    p.table = (const float*)op->table;
+    p.table_R = (float)op->table_R;
+    p.table_len = op->table_len;
+    return p;
+}
+
+// persistent grid: as many CTAs as fit on the device at once (capped by the number of items)
+template <typename Kern> int x_grid_size(Kern kern, int threads, size_t smem, int n_items, int warps, int* out) {
+    int dev = 0, sms = 0, per_sm = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem));
+    if (per_sm < 1) per_sm = 1;
+    int g = sms * per_sm;
+    const int need = (n_items + warps - 1) / warps;
+    if (g > need) g = need;
+    if (g < 1) g = 1;
+    *out = g;
+    return PURIFY_OK;
+}
+
+template <int J, int DEG> int launch_degrid_x_t(purify_op* op, void* y, bool caller_order, cudaStream_t st) {
+    typedef pk::XCfg<J> Cfg;
+    if (op->n_items == 0) return PURIFY_OK;
+    const size_t smem = (size_t)Cfg::WARPS * Cfg::REGION_BYTES + Cfg::WARPS * sizeof(uint64_t);
+    const pk::XParams p = make_xparams(op, caller_order);
+    CK(cudaMemsetAsync(op->x_counter, 0, sizeof(unsigned), st));
+#define LAUNCH_DX(MODE, CALLER)                                                                          \
+    do {                                                                                                 \
+        auto kern = pk::degrid_x_kernel<J, DEG, MODE, CALLER>;                                           \
+        int g = 0;                                                                                       \
+        RUNX(x_grid_size(kern, Cfg::THREADS, smem, op->n_items, Cfg::WARPS, &g));                        \
+        kern<<<g, Cfg::THREADS, smem, st>>>(op->tmap_x, p, (float2*)y);                                  \
+    } while (0)
+#define RUNX(expr) do { int rc_ = (expr); if (rc_) return rc_; } while (0)
+    const bool table = op->mode == PURIFY_KERNEL_TABLE;
+    if (!table && !caller_order) LAUNCH_DX(0, 0);
+    else if (!table && caller_order) LAUNCH_DX(0, 1);
+    else if (table && !caller_order) LAUNCH_DX(1, 0);
+    else LAUNCH_DX(1, 1);
+#undef LAUNCH_DX
+    op->launches++;
+    CK(cudaGetLastError());
+    return PURIFY_OK;
+}
+
+template <int J, int DEG> int launch_grid_x_t(purify_op* op, const void* y, bool caller_order, cudaStream_t st) {
+    typedef pk::XCfg<J> Cfg;
+    if (op->n_items == 0) return PURIFY_OK;
+    const size_t smem = (size_t)Cfg::WARPS * Cfg::REGION_BYTES;
+    const pk::XParams p = make_xparams(op, caller_order);
+    CK(cudaMemsetAsync(op->x_counter, 0, sizeof(unsigned), st));
+#define LAUNCH_GX(MODE, CALLER)                                                                          \
+    do {                                                                                                 \
+        auto kern = pk::grid_x_kernel<J, DEG, MODE, CALLER>;                                             \
+        int g = 0;                                                                                       \
+        RUNX(x_grid_size(kern, Cfg::THREADS, smem, op->n_items, Cfg::WARPS, &g));                        \
+        kern<<<g, Cfg::THREADS, smem, st>>>(p, (const float2*)y);                                        \
+    } while (0)
+    const bool table = op->mode == PURIFY_KERNEL_TABLE;
+    if (!table && !caller_order) LAUNCH_GX(0, 0);
+    else if (!table && caller_order) LAUNCH_GX(0, 1);
+    else if (table && !caller_order) LAUNCH_GX(1, 0);
+    else LAUNCH_GX(1, 1);
+#undef LAUNCH_GX
+#undef RUNX
+    op->launches++;
+    CK(cudaGetLastError());
+    return PURIFY_OK;
+}
+
 int launch_degrid(purify_op* op, void* y, bool caller_order, cudaStream_t st) {
     StageTimer t(op, PURIFY_STAGE_DEGRID, st);
+    if (op->batched) {
+        switch (op->J) {
+            case 4: return launch_degrid_x_t<4, deg_c64(4)>(op, y, caller_order, st);
+            case 6: return launch_degrid_x_t<6, deg_c64(6)>(op, y, caller_order, st);
+            default: return launch_degrid_x_t<8, deg_c64(8)>(op, y, caller_order, st);
+        }
+    }
     if (op->dtype == PURIFY_C64) {
         switch (op->J) {
             case 4: return launch_degrid_t<float, 4, deg_c64(4)>(op, y, caller_order, st);
@@ -197,6 +302,13 @@ int launch_grid(purify_op* op, const void* y, bool caller_order, cudaStream_t st
         CK(cudaMemsetAsync(op->grid, 0, csize(op) * (size_t)op->K * op->K, st));
     }
     StageTimer t(op, PURIFY_STAGE_GRID, st);
+    if (op->batched) {
+        switch (op->J) {
+            case 4: return launch_grid_x_t<4, deg_c64(4)>(op, y, caller_order, st);
+            case 6: return launch_grid_x_t<6, deg_c64(6)>(op, y, caller_order, st);
+            default: return launch_grid_x_t<8, deg_c64(8)>(op, y, caller_order, st);
+        }
+    }
     if (op->dtype == PURIFY_C64) {
         switch (op->J) {
             case 4: return launch_grid_t<float, 4, deg_c64(4)>(op, y, caller_order, st);
@@ -251,11 +363,11 @@ int launch_fft(purify_op* op, int dir, cudaStream_t st) {
 
 int launch_permute(purify_op* op, const void* in, void* out, int to_native, cudaStream_t st) {
     StageTimer t(op, PURIFY_STAGE_PERMUTE, st);
-    if (op->M == 0) return PURIFY_OK;
+    if (op->M_native == 0) return PURIFY_OK;
     if (op->dtype == PURIFY_C64)
-        pk::permute_kernel<float2><<<grid_for(op->M, 256, 148 * 32), 256, 0, st>>>((const float2*)in, (float2*)out, op->perm, op->M, to_native);
+        pk::permute_kernel<float2><<<grid_for(op->M_native, 256, 148 * 32), 256, 0, st>>>((const float2*)in, (float2*)out, op->perm, op->M_native, to_native);
     else
-        pk::permute_kernel<double2><<<grid_for(op->M, 256, 148 * 32), 256, 0, st>>>((const double2*)in, (double2*)out, op->perm, op->M, to_native);
+        pk::permute_kernel<double2><<<grid_for(op->M_native, 256, 148 * 32), 256, 0, st>>>((const double2*)in, (double2*)out, op->perm, op->M_native, to_native);
     op->launches++;
     CK(cudaGetLastError());
     return PURIFY_OK;
@@ -397,6 +509,136 @@ int build_bins(purify_op* op, const void* uv_dev, const void* w_dev, cudaStream_
     return PURIFY_OK;
 }
 
+// a0 for complex64: the batched layout of batched.cuh (device radix sort on band/cell id, per-band
+// batch construction, slot fill).
+int build_bins_x(purify_op* op, const void* uv_dev, const void* w_dev, cudaStream_t st) {
+    const long long M = op->M;
+    const int K = op->K;
+    const int nbx = (K + pk::XBW - 1) / pk::XBW, nby = (K + pk::XBH - 1) / pk::XBH;
+    const int n_bands = nbx * nby;
+    const int boxw = pk::XBW + op->J;
+    op->n_bands = n_bands;
+    op->ntx = nbx;
+    op->n_tiles = n_bands;
+    op->batched = true;
+
+    unsigned *keys = nullptr, *keys2 = nullptr, *idx = nullptr, *perm0 = nullptr, *band_start = nullptr;
+    unsigned *a_nb = nullptr, *a_it = nullptr, *a_items = nullptr, *o_nb = nullptr, *o_it = nullptr, *o_items = nullptr;
+    unsigned *lsrc = nullptr, *nonempty = nullptr;
+    pk::BandTotals* totals = nullptr;
+    int* bad = nullptr;
+    void *cub_tmp = nullptr, *scan_tmp = nullptr;
+    auto cleanup = [&]() {
+        cudaFree(keys); cudaFree(keys2); cudaFree(idx); cudaFree(perm0); cudaFree(band_start); cudaFree(a_nb);
+        cudaFree(a_it); cudaFree(a_items); cudaFree(o_nb); cudaFree(o_it); cudaFree(o_items); cudaFree(lsrc);
+        cudaFree(nonempty); cudaFree(totals); cudaFree(bad); cudaFree(cub_tmp); cudaFree(scan_tmp);
+    };
+#define CKC(call)                                                                                       \
+    do {                                                                                                \
+        cudaError_t e_ = (call);                                                                        \
+        if (e_ != cudaSuccess) {                                                                        \
+            cleanup();                                                                                  \
+            cudaGetLastError();                                                                         \
+            return fail(e_ == cudaErrorMemoryAllocation ? PURIFY_ERR_ALLOC : PURIFY_ERR_CUDA,          \
+                        "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__);    \
+        }                                                                                               \
+    } while (0)
+    const size_t Mz = M > 0 ? (size_t)M : 1, nb1 = (size_t)n_bands + 1;
+    CKC(cudaMalloc(&keys, sizeof(unsigned) * Mz));
+    CKC(cudaMalloc(&keys2, sizeof(unsigned) * Mz));
+    CKC(cudaMalloc(&idx, sizeof(unsigned) * Mz));
+    CKC(cudaMalloc(&perm0, sizeof(unsigned) * Mz));
+    CKC(cudaMalloc(&band_start, sizeof(unsigned) * nb1));
+    CKC(cudaMalloc(&totals, sizeof(pk::BandTotals) * nb1));
+    CKC(cudaMalloc(&a_nb, sizeof(unsigned) * nb1));
+    CKC(cudaMalloc(&a_it, sizeof(unsigned) * nb1));
+    CKC(cudaMalloc(&a_items, sizeof(unsigned) * nb1));
+    CKC(cudaMalloc(&o_nb, sizeof(unsigned) * nb1));
+    CKC(cudaMalloc(&o_it, sizeof(unsigned) * nb1));
+    CKC(cudaMalloc(&o_items, sizeof(unsigned) * nb1));
+    CKC(cudaMalloc(&nonempty, sizeof(unsigned)));
+    CKC(cudaMalloc(&bad, sizeof(int)));
+    CKC(cudaMemsetAsync(bad, 0, sizeof(int), st));
+    CKC(cudaMemsetAsync(nonempty, 0, sizeof(unsigned), st));
+
+    if (M > 0) {
+        pk::xkey_kernel<<<grid_for(M, 256), 256, 0, st>>>((const float2*)uv_dev, M, K, nbx, keys, idx, bad);
+        CKC(cudaGetLastError());
+        int h_bad = 0;
+        CKC(cudaMemcpyAsync(&h_bad, bad, sizeof(int), cudaMemcpyDeviceToHost, st));
+        CKC(cudaStreamSynchronize(st));
+        if (h_bad) {
+            cleanup();
+            return fail(PURIFY_ERR_UV_NONFINITE, "uv contains NaN, Inf or |coordinate| >= 2^30");
+        }
+        int bits = 1;
+        while (bits < 32 && (1ull << bits) < (unsigned long long)n_bands * pk::XCELLS) ++bits;
+        size_t tmp_bytes = 0;
+        CKC(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys, keys2, idx, perm0, (int)M, 0, bits, st));
+        CKC(cudaMalloc(&cub_tmp, tmp_bytes ? tmp_bytes : 16));
+        CKC(cub::DeviceRadixSort::SortPairs(cub_tmp, tmp_bytes, keys, keys2, idx, perm0, (int)M, 0, bits, st));
+    }
+    pk::band_start_kernel<<<(n_bands + 1 + 255) / 256, 256, 0, st>>>(keys2, M, n_bands, band_start);
+    CKC(cudaGetLastError());
+    pk::band_build_kernel<1><<<n_bands, pk::XCELLS, 0, st>>>(keys2, band_start, nbx, boxw, totals, nullptr, nullptr, nullptr,
+                                                             nullptr, nullptr, nullptr, nullptr);
+    CKC(cudaGetLastError());
+    pk::split_totals_kernel<<<(n_bands + 1 + 255) / 256, 256, 0, st>>>(totals, n_bands, a_nb, a_it, a_items, nonempty);
+    CKC(cudaGetLastError());
+    {
+        size_t tmp2 = 0;
+        CKC(cub::DeviceScan::ExclusiveSum(nullptr, tmp2, a_nb, o_nb, n_bands + 1, st));
+        CKC(cudaMalloc(&scan_tmp, tmp2 ? tmp2 : 16));
+        CKC(cub::DeviceScan::ExclusiveSum(scan_tmp, tmp2, a_nb, o_nb, n_bands + 1, st));
+        CKC(cub::DeviceScan::ExclusiveSum(scan_tmp, tmp2, a_it, o_it, n_bands + 1, st));
+        CKC(cub::DeviceScan::ExclusiveSum(scan_tmp, tmp2, a_items, o_items, n_bands + 1, st));
+    }
+    unsigned h_tot[4] = {0, 0, 0, 0};
+    CKC(cudaMemcpyAsync(&h_tot[0], o_nb + n_bands, sizeof(unsigned), cudaMemcpyDeviceToHost, st));
+    CKC(cudaMemcpyAsync(&h_tot[1], o_it + n_bands, sizeof(unsigned), cudaMemcpyDeviceToHost, st));
+    CKC(cudaMemcpyAsync(&h_tot[2], o_items + n_bands, sizeof(unsigned), cudaMemcpyDeviceToHost, st));
+    CKC(cudaMemcpyAsync(&h_tot[3], nonempty, sizeof(unsigned), cudaMemcpyDeviceToHost, st));
+    CKC(cudaStreamSynchronize(st));
+    op->n_batches = h_tot[0];
+    op->M_native = (long long)h_tot[1] * 32;
+    op->n_items = (int)h_tot[2];
+    op->n_bands_nonempty = (int)h_tot[3];
+    op->n_tiles_nonempty = (int)h_tot[3];
+    int rc;
+    const size_t S = op->M_native > 0 ? (size_t)op->M_native : 1, NBz = op->n_batches > 0 ? op->n_batches : 1;
+    if ((rc = dev_alloc(op, &op->uv_s, sizeof(float2) * S))) { cleanup(); return rc; }
+    if ((rc = dev_alloc(op, &op->w_s, sizeof(float) * S))) { cleanup(); return rc; }
+    if ((rc = dev_alloc(op, (void**)&op->perm, sizeof(unsigned) * S))) { cleanup(); return rc; }
+    if ((rc = dev_alloc(op, (void**)&op->x_bhdr, sizeof(uint2) * NBz))) { cleanup(); return rc; }
+    if ((rc = dev_alloc(op, (void**)&op->x_blane, sizeof(unsigned) * 32 * NBz))) { cleanup(); return rc; }
+    if ((rc = dev_alloc(op, (void**)&op->x_items, sizeof(pk::XItem) * (size_t)(op->n_items > 0 ? op->n_items : 1)))) { cleanup(); return rc; }
+    if ((rc = dev_alloc(op, (void**)&op->x_counter, sizeof(unsigned)))) { cleanup(); return rc; }
+    CKC(cudaMalloc(&lsrc, sizeof(unsigned) * 32 * NBz));
+    if (op->n_batches > 0) {
+        pk::band_build_kernel<2><<<n_bands, pk::XCELLS, 0, st>>>(keys2, band_start, nbx, boxw, nullptr, o_nb, o_it, o_items,
+                                                                 op->x_bhdr, op->x_blane, lsrc, op->x_items);
+        CKC(cudaGetLastError());
+        pk::slot_fill_kernel<<<grid_for((long long)op->n_batches * 32, 256), 256, 0, st>>>(
+            op->x_bhdr, op->x_blane, lsrc, op->n_batches, perm0, (const float2*)uv_dev, (const float*)w_dev, K,
+            op->perm, (float2*)op->uv_s, (float*)op->w_s);
+        CKC(cudaGetLastError());
+    }
+    CKC(cudaStreamSynchronize(st));
+    // statistics: fullest band
+    {
+        std::vector<unsigned> bsv(nb1);
+        CKC(cudaMemcpy(bsv.data(), band_start, sizeof(unsigned) * nb1, cudaMemcpyDeviceToHost));
+        op->max_tile_count = 0;
+        for (int b = 0; b < n_bands; ++b) {
+            const long long c = (long long)bsv[b + 1] - (long long)bsv[b];
+            if (c > op->max_tile_count) op->max_tile_count = c;
+        }
+    }
+    cleanup();
+#undef CKC
+    return PURIFY_OK;
+}
+
 template <typename R>
 int build_tables(purify_op* op, cudaStream_t st) {
     int rc;
@@ -439,6 +681,21 @@ int build_tmap(purify_op* op) {
         return fail(PURIFY_ERR_CUDA, "cuTensorMapEncodeTiled entry point not available");
     const int BOX = pk::TILE + op->J;
     const bool f32 = op->dtype == PURIFY_C64;
+    if (op->batched) {
+        const cuuint64_t dims[2] = {(cuuint64_t)2 * op->K, (cuuint64_t)op->K};
+        const cuuint64_t strides[1] = {(cuuint64_t)op->K * csize(op)};
+        const cuuint32_t box[2] = {(cuuint32_t)(2 * (pk::XBW + op->J)), (cuuint32_t)(pk::XBH + op->J - 1)};
+        const cuuint32_t estr[2] = {1, 1};
+        if (box[0] > (cuuint32_t)2 * op->K || box[1] > (cuuint32_t)op->K) {       // grid smaller than one box: no interior band
+            memset(&op->tmap_x, 0, sizeof(op->tmap_x));
+            return PURIFY_OK;
+        }
+        CUresult r = ((EncodeTiledFn)fn)(&op->tmap_x, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, op->grid, dims, strides, box, estr,
+                                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                         CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return fail(PURIFY_ERR_CUDA, "cuTensorMapEncodeTiled (band box) failed: CUresult %d", (int)r);
+        return PURIFY_OK;
+    }
     const cuuint64_t dims[2] = {(cuuint64_t)2 * op->K, (cuuint64_t)op->K};            // inner extent in reals
     const cuuint64_t strides[1] = {(cuuint64_t)op->K * csize(op)};                     // row pitch, bytes
     const cuuint32_t box[2] = {(cuuint32_t)(2 * BOX), (cuuint32_t)BOX};
@@ -500,7 +757,12 @@ int create_impl(purify_op** out, int n, int oversample, int J, long long M, cons
 
     rc = dev_alloc(op, &op->grid, csize(op) * (size_t)op->K * op->K);
     if (rc) return bail(rc);
-    rc = dtype == PURIFY_C64 ? build_bins<float>(op, uv_dev, w_dev, st) : build_bins<double>(op, uv_dev, w_dev, st);
+    if (dtype == PURIFY_C64) {
+        rc = build_bins_x(op, uv_dev, w_dev, st);
+    } else {
+        rc = build_bins<double>(op, uv_dev, w_dev, st);
+        op->M_native = M;
+    }
     if (rc) return bail(rc);
     rc = dtype == PURIFY_C64 ? build_tables<float>(op, st) : build_tables<double>(op, st);
     if (rc) return bail(rc);
@@ -559,6 +821,7 @@ int purify_op_destroy(purify_op* op) {
     if (!op) return PURIFY_OK;
     cudaFree(op->grid); cudaFree(op->uv_s); cudaFree(op->w_s); cudaFree(op->perm); cudaFree(op->items);
     cudaFree(op->corr); cudaFree(op->table); cudaFree(op->y_ws); cudaFree(op->x_ws); cudaFree(op->y_ws2);
+    cudaFree(op->x_bhdr); cudaFree(op->x_blane); cudaFree(op->x_items); cudaFree(op->x_counter);
     if (op->plan_ok) cufftDestroy(op->plan);
     if (op->ev_ok) for (int i = 0; i < 2 * PURIFY_STAGE_COUNT; ++i) cudaEventDestroy(op->ev[i]);
     cudaGetLastError();
@@ -573,6 +836,8 @@ int purify_op_info(const purify_op* op, purify_info* info) {
     info->table_samples_per_unit = op->table_R; info->M = op->M; info->tile = pk::TILE; info->n_tiles = op->n_tiles;
     info->n_tiles_nonempty = op->n_tiles_nonempty; info->n_items = op->n_items; info->poly_degree = op->poly_degree;
     info->poly_max_abs_err = op->poly_err; info->device_bytes = op->device_bytes; info->max_tile_count = op->max_tile_count;
+    info->M_native = op->M_native; info->n_batches = (long long)op->n_batches; info->layout = op->batched ? 1 : 0;
+    if (op->batched) { info->tile = pk::XBW; info->tile_h = pk::XBH; } else { info->tile_h = pk::TILE; }
     return PURIFY_OK;
 }
 
@@ -625,7 +890,7 @@ int purify_normal(purify_op* op, const void* x_in_dev, void* x_out_dev, void* cu
     NEED_OP(op); NEED_PTR(x_in_dev, "x_in"); NEED_PTR(x_out_dev, "x_out");
     begin_call(op);
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    RUN(ensure_ws(op, &op->y_ws, csize(op) * (size_t)op->M));
+    RUN(ensure_ws(op, &op->y_ws, csize(op) * (size_t)op->M_native));
     RUN(degrid_impl(op, x_in_dev, op->y_ws, false, st));
     RUN(grid_impl(op, op->y_ws, x_out_dev, false, st));
     return PURIFY_OK;
@@ -678,7 +943,7 @@ int purify_normal_host(purify_op* op, const void* x_in_host, void* x_out_host, v
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t xb = csize(op) * (size_t)op->n * op->n;
     RUN(ensure_ws(op, &op->x_ws, xb));
-    RUN(ensure_ws(op, &op->y_ws, csize(op) * (size_t)op->M));
+    RUN(ensure_ws(op, &op->y_ws, csize(op) * (size_t)op->M_native));
     CK(cudaMemcpyAsync(op->x_ws, x_in_host, xb, cudaMemcpyHostToDevice, st));
     RUN(degrid_impl(op, op->x_ws, op->y_ws, false, st));
     RUN(grid_impl(op, op->y_ws, op->x_ws, false, st));

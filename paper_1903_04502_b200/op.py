@@ -38,7 +38,8 @@ class PurifyInfo(C.Structure):
     _fields_ = [("n", C.c_int), ("K", C.c_int), ("J", C.c_int), ("dtype", C.c_int), ("kernel_mode", C.c_int),
                 ("table_samples_per_unit", C.c_int), ("M", C.c_longlong), ("tile", C.c_int), ("n_tiles", C.c_int),
                 ("n_tiles_nonempty", C.c_int), ("n_items", C.c_int), ("poly_degree", C.c_int),
-                ("poly_max_abs_err", C.c_double), ("device_bytes", C.c_longlong), ("max_tile_count", C.c_longlong)]
+                ("poly_max_abs_err", C.c_double), ("device_bytes", C.c_longlong), ("max_tile_count", C.c_longlong),
+                ("M_native", C.c_longlong), ("n_batches", C.c_longlong), ("layout", C.c_int), ("tile_h", C.c_int)]
 
 
 class PurifyError(RuntimeError):
@@ -123,6 +124,7 @@ class PurifyOp:
                 C.c_void_p(w.data_ptr()) if w is not None and M > 0 else None,
                 int(dtype), C.byref(opts), _stream())
         _check(st, "purify_op_create")
+        self.M_native = int(self.info()["M_native"])      # length of native-order vectors (>= M)
 
     # -- lifetime
     def close(self):
@@ -149,13 +151,16 @@ class PurifyOp:
         return {k: getattr(inf, k) for k, _ in PurifyInfo._fields_}
 
     def permutation(self) -> torch.Tensor:
-        """native -> caller index, as an int64 tensor on the device (copy)."""
+        """native -> caller index, as an int64 tensor of M_native entries on the device (copy);
+        -1 marks a padding entry of the complex64 layout."""
         p = C.c_void_p()
         _check(self._L.purify_op_permutation(self._h, C.byref(p)), "purify_op_permutation")
-        if self.M == 0:
+        if self.M_native == 0:
             return torch.empty(0, dtype=torch.int64, device="cuda")
-        view = torch.as_tensor(_DeviceArray(p.value, self.M, "<i4"), device="cuda")   # zero-copy view
-        return view.to(torch.int64) & 0xFFFFFFFF
+        view = torch.as_tensor(_DeviceArray(p.value, self.M_native, "<i4"), device="cuda")   # zero-copy view
+        out = view.to(torch.int64) & 0xFFFFFFFF
+        out[out == 0xFFFFFFFF] = -1
+        return out
 
     def stage_times_ms(self) -> dict:
         arr = (C.c_float * 8)()
@@ -171,16 +176,17 @@ class PurifyOp:
             raise ValueError(f"{name} must be a contiguous {self.n}x{self.n} {_CDT[self.dtype]} tensor")
         return C.c_void_p(x.data_ptr())
 
-    def _y(self, y, name="y"):
-        if y.dtype != _CDT[self.dtype] or y.numel() != self.M or not y.is_contiguous():
-            raise ValueError(f"{name} must be a contiguous [{self.M}] {_CDT[self.dtype]} tensor")
-        return C.c_void_p(y.data_ptr()) if self.M > 0 else None
+    def _y(self, y, name="y", native=False):
+        m = self.M_native if native else self.M
+        if y.dtype != _CDT[self.dtype] or y.numel() != m or not y.is_contiguous():
+            raise ValueError(f"{name} must be a contiguous [{m}] {_CDT[self.dtype]} tensor")
+        return C.c_void_p(y.data_ptr()) if m > 0 else None
 
     def _new_x(self, device="cuda"):
         return torch.empty((self.n, self.n), dtype=_CDT[self.dtype], device=device)
 
-    def _new_y(self, device="cuda"):
-        return torch.empty(self.M, dtype=_CDT[self.dtype], device=device)
+    def _new_y(self, device="cuda", native=False):
+        return torch.empty(self.M_native if native else self.M, dtype=_CDT[self.dtype], device=device)
 
     @staticmethod
     def _dev(*ts):
@@ -190,17 +196,17 @@ class PurifyOp:
 
     # -- Phi, Phi^dagger, Phi^dagger Phi (device buffers)
     def degrid(self, x, y=None, native=False):
-        y = self._new_y() if y is None else y
+        y = self._new_y(native=native) if y is None else y
         self._dev(x, y)
         fn = self._L.purify_degrid_native if native else self._L.purify_degrid
-        _check(fn(self._h, self._x(x), self._y(y), _stream()), "purify_degrid")
+        _check(fn(self._h, self._x(x), self._y(y, native=native), _stream()), "purify_degrid")
         return y
 
     def grid(self, y, x=None, native=False):
         x = self._new_x() if x is None else x
         self._dev(x, y)
         fn = self._L.purify_grid_native if native else self._L.purify_grid
-        _check(fn(self._h, self._y(y), self._x(x), _stream()), "purify_grid")
+        _check(fn(self._h, self._y(y, native=native), self._x(x), _stream()), "purify_grid")
         return x
 
     def normal(self, x, out=None):
@@ -210,15 +216,15 @@ class PurifyOp:
         return out
 
     def permute_to_native(self, y, out=None):
-        out = self._new_y() if out is None else out
+        out = self._new_y(native=True) if out is None else out
         self._dev(y, out)
-        _check(self._L.purify_permute_to_native(self._h, self._y(y), self._y(out), _stream()), "permute_to_native")
+        _check(self._L.purify_permute_to_native(self._h, self._y(y), self._y(out, "out", True), _stream()), "permute_to_native")
         return out
 
     def permute_from_native(self, y, out=None):
         out = self._new_y() if out is None else out
         self._dev(y, out)
-        _check(self._L.purify_permute_from_native(self._h, self._y(y), self._y(out), _stream()), "permute_from_native")
+        _check(self._L.purify_permute_from_native(self._h, self._y(y, "y", True), self._y(out), _stream()), "permute_from_native")
         return out
 
     # -- host-buffer (end-to-end) entry points

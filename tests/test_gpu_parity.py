@@ -61,11 +61,14 @@ def run_all_checks(x, uv, w, J, dtype, mode="analytic", R=4096, **kw):
     y_ref = oracle.degrid(x, uv, w, J, **okw)
     y = host(op.degrid(dev(x)))
     assert rel_l2(y, y_ref) <= tol
-    perm = host(op.permutation())
-    assert sorted(perm.tolist()) == list(range(M))
+    perm = host(op.permutation())                          # M_native entries, -1 = padding (complex64 layout)
+    valid = perm >= 0
+    assert len(perm) == op.M_native >= M
+    assert sorted(perm[valid].tolist()) == list(range(M))
     y_nat = host(op.degrid(dev(x), native=True))
-    assert rel_l2(y_nat, y_ref[perm]) <= tol
-    assert np.array_equal(y_nat, y[perm])                   # same numbers, different order
+    assert rel_l2(y_nat[valid], y_ref[perm[valid]]) <= tol
+    assert np.array_equal(y_nat[valid], y[perm[valid]])     # same numbers, different order
+    assert not np.any(y_nat[~valid])                        # padding entries are written as 0
     # stage: Fourier grid in the mathematical layout
     B_ref = oracle.fft2(oracle.pad(x, J), -1)
     assert rel_l2(host(op.stage_fourier_grid(dev(x))), B_ref) <= tol
@@ -74,13 +77,16 @@ def run_all_checks(x, uv, w, J, dtype, mode="analytic", R=4096, **kw):
     img_ref = oracle.grid(yv, uv, w, n, J, **okw)
     img = host(op.grid(dev(yv)))
     assert rel_l2(img, img_ref) <= tol
-    img_nat = host(op.grid(dev(yv[perm]), native=True))
+    yv_nat = np.full(len(perm), np.nan + 1j * np.nan, dtype=yv.dtype)     # padding holds NaN: must be ignored
+    yv_nat[valid] = yv[perm[valid]]
+    img_nat = host(op.grid(dev(yv_nat), native=True))
     assert rel_l2(img_nat, img_ref) <= tol
     Bp_ref = oracle.grid_to_grid(yv, uv, w, 2 * n, J, **okw)
     assert rel_l2(host(op.stage_gridded(dev(yv))), Bp_ref) <= tol
     # permutation helpers
-    assert np.array_equal(host(op.permute_to_native(dev(yv))), yv[perm])
-    assert np.array_equal(host(op.permute_from_native(dev(yv[perm]))), yv)
+    to_nat = host(op.permute_to_native(dev(yv)))
+    assert np.array_equal(to_nat[valid], yv[perm[valid]]) and not np.any(to_nat[~valid])
+    assert np.array_equal(host(op.permute_from_native(dev(yv_nat))), yv)
     # ---- Phi^dagger Phi
     nrm_ref = oracle.grid(y_ref, uv, w, n, J, **okw)
     xin = dev(x)
