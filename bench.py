@@ -282,8 +282,10 @@ def run_ours(args):
     reps = max(3, args.steps // 2)
     ms_phi = timed(lambda: op.degrid(x_dev, y_dev, native=True), reps)
     ms_phit = timed(lambda: op.grid(y_dev, out_dev, native=True), reps)
-    ms_phi_caller = timed(lambda: op.degrid(x_dev, y_dev, native=False), reps)
-    ms_phit_caller = timed(lambda: op.grid(y_dev, out_dev, native=False), reps)
+    y_call = op.permute_from_native(y_dev)
+    ms_phi_caller = timed(lambda: op.degrid(x_dev, y_call, native=False), reps)
+    ms_phit_caller = timed(lambda: op.grid(y_call, out_dev, native=False), reps)
+    del y_call
 
     # ---- end to end through the C ABI with HOST buffers (H2D of x, D2H of the result inside)
     op.normal_host(x_pin, out_pin)
