@@ -44,6 +44,9 @@ template <int J> struct XCfg {
 struct XItem {
     int x0, y0;          // band origin, internal layout
     int begin, end;      // batch range
+    unsigned iter0;      // first iteration (slot / 32) of the item: its slots are one contiguous stream
+    unsigned iters;      // number of iterations (sum of n_iter over the item's batches)
+    int pad0, pad1;
 };
 
 struct XParams {
@@ -217,6 +220,7 @@ band_build_kernel(const unsigned* __restrict__ keys, const unsigned* __restrict_
                 items[item0 + item].x0 = x0;
                 items[item0 + item].y0 = y0;
                 items[item0 + item].begin = (int)(nb0 + b);
+                items[item0 + item].iter0 = it0 + excl;
                 if (item > 0) items[item0 + item - 1].end = (int)(nb0 + b);
             }
             if (b == NB - 1) items[item0 + item].end = (int)(nb0 + NB);
@@ -366,37 +370,101 @@ __device__ __forceinline__ unsigned x_next_item(unsigned* counter, int lane) {
     return __shfl_sync(0xffffffffu, it, 0);
 }
 
+// a0.5: iteration count of every item (its slots are one contiguous stream of `iters` x 32 slots).
+__global__ void item_iters_kernel(XItem* __restrict__ items, int n_items, const uint2* __restrict__ bhdr) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_items) return;
+    const uint2 h = bhdr[items[i].end - 1];
+    items[i].iters = h.x + (h.y & 0xFFFFu) - items[i].iter0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Visibility stream ring.  The slots of one item are contiguous in HBM, so every warp streams them
+// through a private ring of S stages in shared memory, each filled by 1-D bulk copies
+// (cp.async.bulk, mbarrier completion) of CH iterations (CH x 32 slots): uv, w and - for the
+// adjoint - y.  The copies run S-1 chunks ahead of the arithmetic, which is what hides the HBM
+// latency (profiles/r1b_summary.md: with a one-deep register prefetch both kernels were
+// long-scoreboard bound at 32 % issue utilisation).
+__device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(smem_dst)), "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+template <int CH, bool WITH_Y> struct RingCfg {
+    static constexpr int UV = CH * 256, W = CH * 128, Y = WITH_Y ? CH * 256 : 0;
+    static constexpr int STAGE = UV + W + Y;
+};
+
+template <int J, int CH, int S, bool WITH_Y> struct XSmem {
+    static constexpr int WARP_BYTES = XCfg<J>::REGION_BYTES + S * RingCfg<CH, WITH_Y>::STAGE;
+    static constexpr int BARS = S + 1;                   // per warp: ring stages + the box
+    static constexpr size_t TOTAL = (size_t)XCfg<J>::WARPS * WARP_BYTES + XCfg<J>::WARPS * BARS * sizeof(uint64_t);
+};
+
+// lane 0: start the copies of chunk c (iterations [c CH, c CH + n)) of the item into `stage`
+template <int CH, bool WITH_Y>
+__device__ __forceinline__ void ring_issue(unsigned char* ring, uint64_t* rbar, int stage, const XParams& p,
+                                           const float2* y, unsigned iter0, int c, int T) {
+    typedef RingCfg<CH, WITH_Y> R;
+    const int n = min(CH, T - c * CH);
+    const size_t s0 = ((size_t)iter0 + (size_t)c * CH) * 32;
+    unsigned char* st = ring + stage * R::STAGE;
+    fence_proxy_async();
+    mbar_expect_tx(rbar + stage, (uint32_t)(n * (256 + 128 + (WITH_Y ? 256 : 0))));
+    bulk_g2s(st, p.uv + s0, (uint32_t)(n * 256), rbar + stage);
+    bulk_g2s(st + R::UV, p.w + s0, (uint32_t)(n * 128), rbar + stage);
+    if (WITH_Y) bulk_g2s(st + R::UV + R::W, y + s0, (uint32_t)(n * 256), rbar + stage);
+}
+
 // ---------------------------------------------------------------------------------------------
 // a3 (complex64): W G.  Persistent warps; per item the band's box is staged by one TMA load into the
-// warp's private shared-memory region; per batch every lane loads its cell's J x J patch into
-// registers (conflict-free 8-byte loads) and then runs its unit's visibilities out of registers.
-// HBM per slot: uv 8 + w 4 read, y 8 written (+ perm 4 and a scattered 8-byte store in caller order).
-template <int J, int DEG, int MODE, int CALLER>
+// warp's private shared-memory region and the item's visibility stream runs through the warp's ring;
+// per batch every lane loads its cell's J x J patch into registers and then runs its unit's
+// visibilities out of registers.  HBM per slot: uv 8 + w 4 read, y 8 written (native order).
+template <int J, int DEG, int MODE, int CH, int S>
 __global__ void __launch_bounds__(XCfg<J>::THREADS)
 degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float2* __restrict__ y) {
     typedef XCfg<J> Cfg;
+    typedef RingCfg<CH, false> R;
+    typedef XSmem<J, CH, S, false> SM;
     constexpr int BOXW = Cfg::BOXW, BOXH = Cfg::BOXH, XOFF = Cfg::XOFF;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    float2* tile = reinterpret_cast<float2*>(smem_raw + warp * Cfg::REGION_BYTES);
-    uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + Cfg::WARPS * Cfg::REGION_BYTES) + warp;
-    if (lane == 0) { mbar_init(bar, 1); fence_barrier_init(); }
+    float2* tile = reinterpret_cast<float2*>(smem_raw + warp * SM::WARP_BYTES);
+    unsigned char* ring = smem_raw + warp * SM::WARP_BYTES + Cfg::REGION_BYTES;
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + Cfg::WARPS * SM::WARP_BYTES) + warp * SM::BARS;
+    uint64_t* rbar = bar + 1;
+    if (lane == 0) {
+        for (int i = 0; i < SM::BARS; ++i) mbar_init(bar + i, 1);
+        fence_barrier_init();
+    }
     __syncwarp();
-    uint32_t phase = 0;
+    uint32_t box_phase = 0, ring_phase = 0;
+    int stage = 0;
 
     for (unsigned item = x_next_item(p.counter, lane); item < (unsigned)p.n_items; item = x_next_item(p.counter, lane)) {
         const XItem it = p.items[item];
+        const int T = (int)it.iters, nch = (T + CH - 1) / CH;
         const int bx0 = it.x0 - (J / 2 - 1) - XOFF, by0 = it.y0 - (J / 2 - 1);
         const bool interior = bx0 >= 0 && by0 >= 0 && bx0 + BOXW <= p.K && by0 + BOXH <= p.K;
         __syncwarp();                                   // every lane is done with the previous box
-        if (interior) {
-            if (lane == 0) {
+        if (lane == 0) {
+            if (interior) {
                 fence_proxy_async();
                 mbar_expect_tx(bar, (uint32_t)(sizeof(float2) * BOXW * BOXH));
                 tma_load_2d(tile, &tmap, 2 * bx0, by0, bar);
             }
-            mbar_wait(bar, phase);
-            phase ^= 1;
+            int st = stage;
+            for (int c = 0; c < S && c < nch; ++c) {
+                ring_issue<CH, false>(ring, rbar, st, p, nullptr, it.iter0, c, T);
+                st = st + 1 == S ? 0 : st + 1;
+            }
+        }
+        uint2 hn = p.bhdr[it.begin];
+        unsigned lwn = p.blane[(size_t)it.begin * 32 + lane];
+        if (interior) {
+            mbar_wait(bar, box_phase);
+            box_phase ^= 1;
         } else {
             for (int i = lane; i < BOXW * BOXH; i += 32) {
                 const int r = wrap_idx(by0 + i / BOXW, p.K, p.kmask), c = wrap_idx(bx0 + i % BOXW, p.K, p.kmask);
@@ -404,9 +472,12 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
             }
             __syncwarp();
         }
+        int gi = 0;                                     // iteration within the item
+        float2* yout = y + (size_t)it.iter0 * 32 + lane;
         for (int b = it.begin; b < it.end; ++b) {
-            const uint2 h = p.bhdr[b];
-            const unsigned lw = p.blane[(size_t)b * 32 + lane];
+            const uint2 h = hn;
+            const unsigned lw = lwn;
+            if (b + 1 < it.end) { hn = p.bhdr[b + 1]; lwn = p.blane[(size_t)(b + 1) * 32 + lane]; }
             const int n_iter = (int)(h.y & 0xFFFFu);
             const int ly = (lw >> 5) & 15, lx = lw & 31;
             const int cx = it.x0 + lx - p.Kh, cy = it.y0 + ly - p.Kh;       // cell = floor(u'), floor(v')
@@ -419,13 +490,12 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
 #pragma unroll
                     for (int c = 0; c < J; ++c) B[a][c] = src[a * BOXW + c];
             }
-            size_t slot = (size_t)h.x * 32 + lane;
-            float2 uvk = p.uv[slot];
-            float wk = p.w[slot];
-            for (int i = 0; i < n_iter; ++i) {
-                float2 uvn = uvk;
-                float wn = 0.f;
-                if (i + 1 < n_iter) { uvn = p.uv[slot + 32]; wn = p.w[slot + 32]; }
+            for (int i = 0; i < n_iter; ++i, ++gi) {
+                const int off = gi & (CH - 1);
+                if (off == 0) mbar_wait(rbar + stage, ring_phase);
+                const unsigned char* st = ring + stage * R::STAGE;
+                const float2 uvk = reinterpret_cast<const float2*>(st)[off * 32 + lane];
+                const float wk = reinterpret_cast<const float*>(st + R::UV)[off * 32 + lane];
                 float2 g[J];
                 x_weights<J, DEG, MODE>(uvk, cellf, cx, cy, p, g);
                 float2 acc = make_float2(0.f, 0.f);
@@ -436,42 +506,66 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
                     for (int c = 1; c < J; ++c) row = fma2(dup2(g[c].x), B[a][c], row);
                     acc = fma2(dup2(g[a].y), row, acc);
                 }
-                const float2 out = mul2(dup2(wk), acc);                     // padding slots: w = 0 -> 0
-                if (CALLER) {
-                    const unsigned pi = p.perm[slot];
-                    if (pi != PERM_PAD) y[pi] = out;
-                } else {
-                    y[slot] = out;
+                yout[(size_t)gi * 32] = mul2(dup2(wk), acc);                // padding slots: w = 0 -> 0
+                if (off == CH - 1 || gi == T - 1) {                         // chunk consumed: refill its stage
+                    __syncwarp();
+                    const int cn = gi / CH + S;
+                    if (lane == 0 && cn < nch) ring_issue<CH, false>(ring, rbar, stage, p, nullptr, it.iter0, cn, T);
+                    if (++stage == S) { stage = 0; ring_phase ^= 1; }
                 }
-                slot += 32; uvk = uvn; wk = wn;
             }
         }
     }
 }
 
 // ---------------------------------------------------------------------------------------------
-// a4 (complex64): G^dagger W^dagger.  Same items / batches.  Every lane accumulates its unit's
-// J x J outer products in registers; at the end of the batch the accumulators are added into the
-// warp's private shared-memory box (lanes of one pass hold distinct cells => distinct addresses in
-// every step, no atomics; __syncwarp orders the steps because footprints of different lanes overlap);
-// at the end of the item the box is added to the global grid with one 8-byte reduction per non-zero
-// cell (RED.ADD.F32x2; halos of neighbouring bands and the items of one band meet there).
-template <int J, int DEG, int MODE, int CALLER>
+// a4 (complex64): G^dagger W^dagger.  Same items / batches / ring (with y).  Every lane accumulates
+// its unit's J x J outer products in registers; at the end of the batch the accumulators are added
+// into the warp's private shared-memory box (lanes of one pass hold distinct cells => distinct
+// addresses in every step, no atomics; __syncwarp orders the steps because footprints of different
+// lanes overlap); at the end of the item the box is added to the global grid with one 8-byte
+// reduction per non-zero cell (RED.ADD.F32x2; halos of neighbouring bands and the items of one band
+// meet there).
+template <int J, int DEG, int MODE, int CH, int S>
 __global__ void __launch_bounds__(XCfg<J>::THREADS)
 grid_x_kernel(const XParams p, const float2* __restrict__ y) {
     typedef XCfg<J> Cfg;
+    typedef RingCfg<CH, true> R;
+    typedef XSmem<J, CH, S, true> SM;
     constexpr int BOXW = Cfg::BOXW, BOXH = Cfg::BOXH, XOFF = Cfg::XOFF;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    float2* tile = reinterpret_cast<float2*>(smem_raw + warp * Cfg::REGION_BYTES);
+    float2* tile = reinterpret_cast<float2*>(smem_raw + warp * SM::WARP_BYTES);
+    unsigned char* ring = smem_raw + warp * SM::WARP_BYTES + Cfg::REGION_BYTES;
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + Cfg::WARPS * SM::WARP_BYTES) + warp * SM::BARS;
+    uint64_t* rbar = bar + 1;
+    if (lane == 0) {
+        for (int i = 0; i < SM::BARS; ++i) mbar_init(bar + i, 1);
+        fence_barrier_init();
+    }
+    __syncwarp();
+    uint32_t ring_phase = 0;
+    int stage = 0;
 
     for (unsigned item = x_next_item(p.counter, lane); item < (unsigned)p.n_items; item = x_next_item(p.counter, lane)) {
         const XItem it = p.items[item];
+        const int T = (int)it.iters, nch = (T + CH - 1) / CH;
+        if (lane == 0) {
+            int st = stage;
+            for (int c = 0; c < S && c < nch; ++c) {
+                ring_issue<CH, true>(ring, rbar, st, p, y, it.iter0, c, T);
+                st = st + 1 == S ? 0 : st + 1;
+            }
+        }
+        uint2 hn = p.bhdr[it.begin];
+        unsigned lwn = p.blane[(size_t)it.begin * 32 + lane];
         for (int i = lane; i < BOXW * BOXH; i += 32) tile[i] = make_float2(0.f, 0.f);
         __syncwarp();
+        int gi = 0;
         for (int b = it.begin; b < it.end; ++b) {
-            const uint2 h = p.bhdr[b];
-            const unsigned lw = p.blane[(size_t)b * 32 + lane];
+            const uint2 h = hn;
+            const unsigned lw = lwn;
+            if (b + 1 < it.end) { hn = p.bhdr[b + 1]; lwn = p.blane[(size_t)(b + 1) * 32 + lane]; }
             const int n_iter = (int)(h.y & 0xFFFFu);
             const bool two_pass = (h.y >> 16) & 1u;
             const int cnt = (int)(lw >> 16);
@@ -484,29 +578,29 @@ grid_x_kernel(const XParams p, const float2* __restrict__ y) {
 #pragma unroll
                 for (int c = 0; c < J; ++c) A[a][c] = make_float2(0.f, 0.f);
 
-            size_t slot = (size_t)h.x * 32 + lane;
-            auto load_y = [&](size_t s, bool ok) -> float2 {
-                if (!ok) return make_float2(0.f, 0.f);
-                if (CALLER) return y[p.perm[s]];
-                return y[s];
-            };
-            float2 uvk = p.uv[slot];
-            float wk = p.w[slot];
-            float2 yk = load_y(slot, 0 < cnt);
-            for (int i = 0; i < n_iter; ++i) {
-                float2 uvn = uvk, yn = make_float2(0.f, 0.f);
-                float wn = 0.f;
-                if (i + 1 < n_iter) { uvn = p.uv[slot + 32]; wn = p.w[slot + 32]; yn = load_y(slot + 32, i + 1 < cnt); }
+            for (int i = 0; i < n_iter; ++i, ++gi) {
+                const int off = gi & (CH - 1);
+                if (off == 0) mbar_wait(rbar + stage, ring_phase);
+                const unsigned char* st = ring + stage * R::STAGE;
+                const float2 uvk = reinterpret_cast<const float2*>(st)[off * 32 + lane];
+                const float wk = reinterpret_cast<const float*>(st + R::UV)[off * 32 + lane];
+                float2 yk = reinterpret_cast<const float2*>(st + R::UV + R::W)[off * 32 + lane];
+                if (i >= cnt) yk = make_float2(0.f, 0.f);                   // padding slot: whatever y holds there is ignored
                 float2 g[J];
                 x_weights<J, DEG, MODE>(uvk, cellf, cx, cy, p, g);
-                const float2 z = mul2(dup2(wk), yk);                        // padding: w = 0 and y = 0
+                const float2 z = mul2(dup2(wk), yk);
 #pragma unroll
                 for (int a = 0; a < J; ++a) {
                     const float2 q = mul2(dup2(g[a].y), z);
 #pragma unroll
                     for (int c = 0; c < J; ++c) A[a][c] = fma2(dup2(g[c].x), q, A[a][c]);
                 }
-                slot += 32; uvk = uvn; wk = wn; yk = yn;
+                if (off == CH - 1 || gi == T - 1) {
+                    __syncwarp();
+                    const int cn = gi / CH + S;
+                    if (lane == 0 && cn < nch) ring_issue<CH, true>(ring, rbar, stage, p, y, it.iter0, cn, T);
+                    if (++stage == S) { stage = 0; ring_phase ^= 1; }
+                }
             }
             // ---- flush the accumulators into the warp's box.  Idle lanes (no unit) stay out; a batch
             // that holds one cell twice (lanes r and 16 + r) flushes its two half-warps one after the other.

@@ -223,51 +223,46 @@ template <typename Kern> int x_grid_size(Kern kern, int threads, size_t smem, in
     return PURIFY_OK;
 }
 
-template <int J, int DEG> int launch_degrid_x_t(purify_op* op, void* y, bool caller_order, cudaStream_t st) {
+// ring geometry of the complex64 kernels: CH iterations per chunk, S stages (batched.cuh "ring")
+constexpr int X_CH = 4, X_S_DEGRID = 4, X_S_GRID = 3;
+
+template <int J, int DEG> int launch_degrid_x_t(purify_op* op, void* y, cudaStream_t st) {
     typedef pk::XCfg<J> Cfg;
     if (op->n_items == 0) return PURIFY_OK;
-    const size_t smem = (size_t)Cfg::WARPS * Cfg::REGION_BYTES + Cfg::WARPS * sizeof(uint64_t);
-    const pk::XParams p = make_xparams(op, caller_order);
+    const size_t smem = pk::XSmem<J, X_CH, X_S_DEGRID, false>::TOTAL;
+    const pk::XParams p = make_xparams(op, false);
     CK(cudaMemsetAsync(op->x_counter, 0, sizeof(unsigned), st));
-#define LAUNCH_DX(MODE, CALLER)                                                                          \
-    do {                                                                                                 \
-        auto kern = pk::degrid_x_kernel<J, DEG, MODE, CALLER>;                                           \
-        int g = 0;                                                                                       \
-        RUNX(x_grid_size(kern, Cfg::THREADS, smem, op->n_items, Cfg::WARPS, &g));                        \
-        kern<<<g, Cfg::THREADS, smem, st>>>(op->tmap_x, p, (float2*)y);                                  \
-    } while (0)
-#define RUNX(expr) do { int rc_ = (expr); if (rc_) return rc_; } while (0)
-    const bool table = op->mode == PURIFY_KERNEL_TABLE;
-    if (!table && !caller_order) LAUNCH_DX(0, 0);
-    else if (!table && caller_order) LAUNCH_DX(0, 1);
-    else if (table && !caller_order) LAUNCH_DX(1, 0);
-    else LAUNCH_DX(1, 1);
-#undef LAUNCH_DX
+    int g = 0, rc;
+    if (op->mode == PURIFY_KERNEL_TABLE) {
+        auto kern = pk::degrid_x_kernel<J, DEG, 1, X_CH, X_S_DEGRID>;
+        if ((rc = x_grid_size(kern, Cfg::THREADS, smem, op->n_items, Cfg::WARPS, &g))) return rc;
+        kern<<<g, Cfg::THREADS, smem, st>>>(op->tmap_x, p, (float2*)y);
+    } else {
+        auto kern = pk::degrid_x_kernel<J, DEG, 0, X_CH, X_S_DEGRID>;
+        if ((rc = x_grid_size(kern, Cfg::THREADS, smem, op->n_items, Cfg::WARPS, &g))) return rc;
+        kern<<<g, Cfg::THREADS, smem, st>>>(op->tmap_x, p, (float2*)y);
+    }
     op->launches++;
     CK(cudaGetLastError());
     return PURIFY_OK;
 }
 
-template <int J, int DEG> int launch_grid_x_t(purify_op* op, const void* y, bool caller_order, cudaStream_t st) {
+template <int J, int DEG> int launch_grid_x_t(purify_op* op, const void* y, cudaStream_t st) {
     typedef pk::XCfg<J> Cfg;
     if (op->n_items == 0) return PURIFY_OK;
-    const size_t smem = (size_t)Cfg::WARPS * Cfg::REGION_BYTES;
-    const pk::XParams p = make_xparams(op, caller_order);
+    const size_t smem = pk::XSmem<J, X_CH, X_S_GRID, true>::TOTAL;
+    const pk::XParams p = make_xparams(op, false);
     CK(cudaMemsetAsync(op->x_counter, 0, sizeof(unsigned), st));
-#define LAUNCH_GX(MODE, CALLER)                                                                          \
-    do {                                                                                                 \
-        auto kern = pk::grid_x_kernel<J, DEG, MODE, CALLER>;                                             \
-        int g = 0;                                                                                       \
-        RUNX(x_grid_size(kern, Cfg::THREADS, smem, op->n_items, Cfg::WARPS, &g));                        \
-        kern<<<g, Cfg::THREADS, smem, st>>>(p, (const float2*)y);                                        \
-    } while (0)
-    const bool table = op->mode == PURIFY_KERNEL_TABLE;
-    if (!table && !caller_order) LAUNCH_GX(0, 0);
-    else if (!table && caller_order) LAUNCH_GX(0, 1);
-    else if (table && !caller_order) LAUNCH_GX(1, 0);
-    else LAUNCH_GX(1, 1);
-#undef LAUNCH_GX
-#undef RUNX
+    int g = 0, rc;
+    if (op->mode == PURIFY_KERNEL_TABLE) {
+        auto kern = pk::grid_x_kernel<J, DEG, 1, X_CH, X_S_GRID>;
+        if ((rc = x_grid_size(kern, Cfg::THREADS, smem, op->n_items, Cfg::WARPS, &g))) return rc;
+        kern<<<g, Cfg::THREADS, smem, st>>>(p, (const float2*)y);
+    } else {
+        auto kern = pk::grid_x_kernel<J, DEG, 0, X_CH, X_S_GRID>;
+        if ((rc = x_grid_size(kern, Cfg::THREADS, smem, op->n_items, Cfg::WARPS, &g))) return rc;
+        kern<<<g, Cfg::THREADS, smem, st>>>(p, (const float2*)y);
+    }
     op->launches++;
     CK(cudaGetLastError());
     return PURIFY_OK;
@@ -277,9 +272,9 @@ int launch_degrid(purify_op* op, void* y, bool caller_order, cudaStream_t st) {
     StageTimer t(op, PURIFY_STAGE_DEGRID, st);
     if (op->batched) {
         switch (op->J) {
-            case 4: return launch_degrid_x_t<4, deg_c64(4)>(op, y, caller_order, st);
-            case 6: return launch_degrid_x_t<6, deg_c64(6)>(op, y, caller_order, st);
-            default: return launch_degrid_x_t<8, deg_c64(8)>(op, y, caller_order, st);
+            case 4: return launch_degrid_x_t<4, deg_c64(4)>(op, y, st);
+            case 6: return launch_degrid_x_t<6, deg_c64(6)>(op, y, st);
+            default: return launch_degrid_x_t<8, deg_c64(8)>(op, y, st);
         }
     }
     if (op->dtype == PURIFY_C64) {
@@ -304,9 +299,9 @@ int launch_grid(purify_op* op, const void* y, bool caller_order, cudaStream_t st
     StageTimer t(op, PURIFY_STAGE_GRID, st);
     if (op->batched) {
         switch (op->J) {
-            case 4: return launch_grid_x_t<4, deg_c64(4)>(op, y, caller_order, st);
-            case 6: return launch_grid_x_t<6, deg_c64(6)>(op, y, caller_order, st);
-            default: return launch_grid_x_t<8, deg_c64(8)>(op, y, caller_order, st);
+            case 4: return launch_grid_x_t<4, deg_c64(4)>(op, y, st);
+            case 6: return launch_grid_x_t<6, deg_c64(6)>(op, y, st);
+            default: return launch_grid_x_t<8, deg_c64(8)>(op, y, st);
         }
     }
     if (op->dtype == PURIFY_C64) {
@@ -618,6 +613,8 @@ int build_bins_x(purify_op* op, const void* uv_dev, const void* w_dev, cudaStrea
         pk::band_build_kernel<2><<<n_bands, pk::XCELLS, 0, st>>>(keys2, band_start, nbx, boxw, nullptr, o_nb, o_it, o_items,
                                                                  op->x_bhdr, op->x_blane, lsrc, op->x_items);
         CKC(cudaGetLastError());
+        pk::item_iters_kernel<<<(op->n_items + 255) / 256, 256, 0, st>>>(op->x_items, op->n_items, op->x_bhdr);
+        CKC(cudaGetLastError());
         pk::slot_fill_kernel<<<grid_for((long long)op->n_batches * 32, 256), 256, 0, st>>>(
             op->x_bhdr, op->x_blane, lsrc, op->n_batches, perm0, (const float2*)uv_dev, (const float*)w_dev, K,
             op->perm, (float2*)op->uv_s, (float*)op->w_s);
@@ -848,14 +845,27 @@ int purify_op_permutation(const purify_op* op, const unsigned** perm_dev) {
     return PURIFY_OK;
 }
 
+// The complex64 (batched) kernels work in native order only; caller order is one extra permutation
+// pass through the handle's native-order workspace (faster than scattering from inside the kernel).
 static int degrid_impl(purify_op* op, const void* x, void* y, bool caller_order, cudaStream_t st) {
     RUN(launch_pad(op, x, st));
     RUN(launch_fft(op, CUFFT_FORWARD, st));
+    if (op->batched && caller_order) {
+        RUN(ensure_ws(op, &op->y_ws, csize(op) * (size_t)op->M_native));
+        RUN(launch_degrid(op, op->y_ws, false, st));
+        return launch_permute(op, op->y_ws, y, 0, st);
+    }
     RUN(launch_degrid(op, y, caller_order, st));
     return PURIFY_OK;
 }
 
 static int grid_impl(purify_op* op, const void* y, void* x, bool caller_order, cudaStream_t st) {
+    if (op->batched && caller_order) {
+        RUN(ensure_ws(op, &op->y_ws, csize(op) * (size_t)op->M_native));
+        RUN(launch_permute(op, y, op->y_ws, 1, st));
+        y = op->y_ws;
+        caller_order = false;
+    }
     RUN(launch_grid(op, y, caller_order, st));
     RUN(launch_fft(op, CUFFT_INVERSE, st));
     RUN(launch_crop(op, x, st));
@@ -977,7 +987,13 @@ int purify_stage_gridded(purify_op* op, const void* y_dev, void* B_dev, void* cu
     NEED_OP(op); NEED_PTR(B_dev, "B"); if (op->M > 0) NEED_PTR(y_dev, "y");
     begin_call(op);
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    RUN(launch_grid(op, y_dev, true, st));
+    if (op->batched) {
+        RUN(ensure_ws(op, &op->y_ws, csize(op) * (size_t)op->M_native));
+        RUN(launch_permute(op, y_dev, op->y_ws, 1, st));
+        RUN(launch_grid(op, op->y_ws, false, st));
+    } else {
+        RUN(launch_grid(op, y_dev, true, st));
+    }
     return relayout(op, op->grid, B_dev, st);
 }
 
