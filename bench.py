@@ -334,7 +334,8 @@ def run_ours(args):
             "clocks": clocks,
             "setup": {"generate_s": t_gen, "create_s": t_create, "n_items": info["n_items"],
                       "n_tiles_nonempty": info["n_tiles_nonempty"], "max_tile_count": info["max_tile_count"],
-                      "device_bytes": info["device_bytes"]},
+                      "device_bytes": info["device_bytes"], "M_native": info["M_native"],
+                      "padding_ratio": info["M_native"] / max(M, 1), "n_batches": info["n_batches"]},
         }
         if world == 1 and not args.no_cpu_baseline:
             ms = min(args.cpu_sample, M)

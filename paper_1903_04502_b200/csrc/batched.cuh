@@ -5,32 +5,37 @@
 // adjoint additionally pays shared-memory read-modify-writes per visibility.  Here a THREAD OWNS A
 // GRID CELL for a run of visibilities: degridding keeps the cell's J x J patch of the Fourier grid
 // in registers, gridding keeps the J x J accumulators in registers, and the inner loop over the
-// run's visibilities touches no shared memory at all.  The 2J^2 complex x real MACs and the paired
-// Horner chains of the kernel weights are issued as packed fp32 (FFMA2, fma.rn.f32x2, sm_100).
+// run's visibilities touches no grid data in shared memory at all.  The 2J^2 complex x real MACs
+// and the paired Horner chains of the kernel weights are issued as packed fp32 (FFMA2, sm_100).
 //
 // Layout (built once at create):
 //   band   32 x 16 cells of the oversampled grid (internal DC-centred layout); one WARP works on one
 //          band at a time with a private (16+J-1) x (32+J) shared-memory box.
-//   unit   up to UNIT_CAP visibilities of ONE cell (a cell with more is split into several units).
-//   batch  32 units, one per lane, processed in lockstep for n_iter = max count iterations.  The 16
-//          lanes of a half-warp hold cells of 16 different residues (ly*BOXW + lx) mod 16, so the
-//          8-byte shared-memory accesses of a half-warp hit 16 different bank pairs (conflict-free);
-//          the units of a residue class are handed out in descending count order, so the counts in a
-//          batch are nearly equal (lane efficiency 0.8-0.9 for Poisson-like cell counts).
-//   slots  visibility data in "native order": slot = 32*(base32 + i) + lane for iteration i of a
-//          batch - coalesced.  Slots past a unit's count are padding: perm = 0xFFFFFFFF, w = 0,
-//          uv = the cell centre, y_native = 0.
-//   item   a run of batches of one band with at most ITEM_ITERS iterations: the unit of dynamic
-//          scheduling (persistent warps pull items from an atomic counter).
+//   unit   up to UNIT_CAP visibilities of ONE cell.  A cell with c visibilities gives floor(c/CAP)
+//          full units and one remainder unit.
+//   batch  32 consecutive units of the band's unit sequence, one per lane, processed in lockstep for
+//          n_iter = (count of the batch's first unit) iterations.  The sequence is: the full units in
+//          layer-major order (layer j = the j-th full unit of every cell that has one, cells
+//          ascending), then the remainder units by descending count - so counts never increase along
+//          the sequence, the counts inside a batch are nearly equal (padding a few per cent), and two
+//          units of the same cell can only meet in a batch that straddles a layer boundary (flagged:
+//          the adjoint then flushes with shared-memory atomics instead of plain read-modify-writes).
+//   slots  visibility data in "native order": slot = 32*(iter0 + i) + lane for iteration i of a
+//          batch.  Slots past a unit's count are padding: perm = 0xFFFFFFFF, w = 0, uv = the unit's
+//          first visibility, y_native = 0.  The per-slot inputs are stored as one record per
+//          ITERATION: 32 x (u, v) then 32 x w = 384 bytes, so a chunk of iterations is ONE bulk copy.
+//   item   a run of batches of one band with about ITEM_ITERS iterations: the unit of dynamic
+//          scheduling (persistent warps pull items from an atomic counter); its slots are contiguous.
 #pragma once
 #include "kernels.cuh"
 
 namespace pk {
 
 constexpr int XBW = 32, XBH = 16, XCELLS = XBW * XBH;   // band geometry
-constexpr int UNIT_CAP = 64;                            // visibilities per unit (L)
+constexpr int UNIT_CAP = 64;                            // visibilities per unit
 constexpr int ITEM_ITERS = 256;                         // iterations per item
 constexpr unsigned PERM_PAD = 0xFFFFFFFFu;
+constexpr int REC_FLOATS = 96, REC_BYTES = 384;         // per-iteration record: uv[32] | w[32]
 
 template <int J> struct XCfg {
     static constexpr int XOFF = (J / 2 - 1) & 1;        // makes the box's first column even (TMA: 16-byte aligned)
@@ -55,24 +60,14 @@ struct XParams {
     const XItem* items;
     int n_items;
     unsigned* counter;            // dynamic item queue (reset before every launch)
-    const uint2* bhdr;            // per batch: x = base32, y = n_iter | flags << 16 (bit 0: duplicate cell => 2-pass flush)
+    const uint2* bhdr;            // per batch: x = first iteration, y = n_iter | flags << 16 (bit 0: a cell may occur twice)
     const unsigned* blane;        // per batch 32 lane words: cell (ly << 5 | lx) | count << 16
-    const float2* uv;             // slots
-    const float* w;               // slots
-    const unsigned* perm;         // slots -> caller index (PERM_PAD for padding); nullptr = native-order y
+    const float* rec;             // per-iteration records (REC_FLOATS floats each)
     KbCoef<float> coef;
     const float* table;
     float table_R;
     int table_len;
 };
-
-// class (residue) of cell (ly, lx) for box pitch boxw, and the inverse enumeration of a class' 32 members
-__host__ __device__ __forceinline__ int x_class(int ly, int lx, int boxw) { return (ly * boxw + lx) & 15; }
-__host__ __device__ __forceinline__ int x_member_cell(int r, int m, int boxw) {
-    const int ly = m >> 1;
-    const int lx = ((r - ly * boxw) & 15) + 16 * (m & 1);
-    return ly * XBW + lx;
-}
 
 // ---------------------------------------------------------------------------------------------
 // a0.1: reduce (u, v) to the principal period, key = band * 512 + cell (band-major).
@@ -118,8 +113,8 @@ __global__ void band_start_kernel(const unsigned* __restrict__ keys, long long M
 }
 
 // ---------------------------------------------------------------------------------------------
-// a0.2 / a0.3: per-band batch construction.  One CTA of 512 threads per band; thread t <-> (class
-// r = t >> 5, member m = t & 31).  PASS 1 counts batches / iterations / items, PASS 2 (after the
+// a0.2 / a0.3: per-band batch construction.  One CTA of 512 threads per band, thread t <-> cell t
+// (ly = t >> 5, lx = t & 31).  PASS 1 counts batches / iterations / items, PASS 2 (after the
 // exclusive scans over bands) writes batch headers, lane words, unit sources and items.
 struct BandTotals { unsigned nb, iters, items; };
 
@@ -131,60 +126,46 @@ band_build_kernel(const unsigned* __restrict__ keys, const unsigned* __restrict_
                   const unsigned* __restrict__ item_off,                // PASS 2 in (exclusive scans)
                   uint2* __restrict__ bhdr, unsigned* __restrict__ blane, unsigned* __restrict__ lsrc,
                   XItem* __restrict__ items) {
-    __shared__ unsigned s_full[16][32], s_rem[16][32], s_start[16][32];
-    __shared__ unsigned s_F[16], s_R[16], s_maxfull[16];
-    __shared__ unsigned s_remsorted[16][32];
-    __shared__ unsigned s_scan[XCELLS];
-    __shared__ unsigned s_ni[XCELLS];
-    __shared__ unsigned s_carry, s_lastni, s_Q;
+    __shared__ unsigned s_rem[XCELLS], s_remsorted[XCELLS], s_scan[XCELLS], s_ni[XCELLS];
+    __shared__ unsigned s_w[XCELLS / 32];
+    __shared__ unsigned s_F, s_Rn, s_maxfull, s_carry, s_lastni;
 
     const int band = blockIdx.x;
     const unsigned bs = band_start[band], be = band_start[band + 1];
-    const int t = threadIdx.x, r = t >> 5, m = t & 31;
+    const int t = threadIdx.x, warp = t >> 5, lane = t & 31;
     if (bs == be) {
         if (PASS == 1 && t == 0) { totals[band].nb = 0; totals[band].iters = 0; totals[band].items = 0; }
         return;
     }
-    // --- cell counts
-    const int cell = x_member_cell(r, m, boxw);
+    if (t == 0) { s_F = 0; s_Rn = 0; s_maxfull = 0; s_carry = 0; s_lastni = 0; }
+    // --- this cell's visibilities: [start, start + cnt) of the sorted order
+    unsigned start, cnt;
     {
-        const unsigned long long k0 = (unsigned long long)band * XCELLS + cell;
+        const unsigned k0 = (unsigned)band * XCELLS + (unsigned)t;
         unsigned lo = bs, hi = be;
         while (lo < hi) { const unsigned mid = lo + ((hi - lo) >> 1); if (keys[mid] < k0) lo = mid + 1; else hi = mid; }
         unsigned lo2 = lo, hi2 = be;
         while (lo2 < hi2) { const unsigned mid = lo2 + ((hi2 - lo2) >> 1); if (keys[mid] <= k0) lo2 = mid + 1; else hi2 = mid; }
-        const unsigned cnt = lo2 - lo;
-        s_start[r][m] = lo;
-        s_full[r][m] = cnt / UNIT_CAP;
-        s_rem[r][m] = cnt % UNIT_CAP;
+        start = lo;
+        cnt = lo2 - lo;
     }
+    const unsigned myfull = cnt / UNIT_CAP, myrem = cnt % UNIT_CAP;
+    s_rem[t] = myrem;
     __syncthreads();
-    // --- per-class totals and remainder ranks (descending, ties by member index)
-    const unsigned myfull = s_full[r][m], myrem = s_rem[r][m];
-    unsigned rank = 0, F = 0, R = 0, maxfull = 0;
-    for (int q = 0; q < 32; ++q) {
-        const unsigned f = s_full[r][q], e = s_rem[r][q];
-        F += f; R += (e > 0); maxfull = max(maxfull, f);
-        if (e > myrem || (e == myrem && q < m)) ++rank;
+    if (myfull) { atomicAdd(&s_F, myfull); atomicMax(&s_maxfull, myfull); }
+    if (myrem) atomicAdd(&s_Rn, 1u);
+    // rank of the remainder unit: descending count, ties by cell (zeros sort last)
+    unsigned rank = 0;
+    for (int q = 0; q < XCELLS; ++q) {
+        const unsigned e = s_rem[q];
+        rank += (e > myrem || (e == myrem && q < t)) ? 1u : 0u;
     }
-    if (m == 0) { s_F[r] = F; s_R[r] = R; s_maxfull[r] = maxfull; }
-    s_remsorted[r][rank] = myrem;            // ranks are a permutation of 0..31 (zeros sort last)
+    s_remsorted[rank] = myrem;
     __syncthreads();
-    if (t == 0) {
-        unsigned Q = 0;
-        for (int q = 0; q < 16; ++q) Q = max(Q, s_F[q] + s_R[q]);
-        s_Q = Q; s_carry = 0; s_lastni = 0;
-    }
-    __syncthreads();
-    const unsigned Q = s_Q, NB = (Q + 1) >> 1;
-
-    // count of the unit at queue position g of class q
-    auto unit_count = [&](int q, unsigned g) -> unsigned {
-        const unsigned Fq = s_F[q];
-        if (g < Fq) return UNIT_CAP;
-        const unsigned j = g - Fq;
-        return j < 32 ? s_remsorted[q][j] : 0u;
-    };
+    const unsigned F = s_F, Rn = s_Rn, maxfull = s_maxfull;
+    const unsigned Q = F + Rn, NB = (Q + 31) >> 5;
+    // n_iter of batch b = count of its first unit (counts never increase along the sequence)
+    auto batch_iters = [&](unsigned b) -> unsigned { return 32u * b < F ? (unsigned)UNIT_CAP : s_remsorted[32u * b - F]; };
 
     const unsigned nb0 = PASS == 2 ? nb_off[band] : 0, it0 = PASS == 2 ? iter_off[band] : 0,
                    item0 = PASS == 2 ? item_off[band] : 0;
@@ -194,10 +175,7 @@ band_build_kernel(const unsigned* __restrict__ keys, const unsigned* __restrict_
     unsigned total_iters = 0;
     for (unsigned base = 0; base < NB; base += XCELLS) {
         const unsigned b = base + t;
-        unsigned ni = 0;
-        if (b < NB)
-            for (int q = 0; q < 16; ++q) ni = max(ni, max(unit_count(q, 2 * b), unit_count(q, 2 * b + 1)));
-        // block-wide inclusive scan of ni
+        const unsigned ni = b < NB ? batch_iters(b) : 0u;
         s_ni[t] = ni;
         s_scan[t] = ni;
         __syncthreads();
@@ -230,54 +208,66 @@ band_build_kernel(const unsigned* __restrict__ keys, const unsigned* __restrict_
         __syncthreads();
         total_iters = s_carry;
     }
-    if (PASS == 1) {
+    if constexpr (PASS == 1) {
         if (t == 0) {
             totals[band].nb = NB;
             totals[band].iters = total_iters;
             // items = distinct values of floor(excl(b) / ITEM_ITERS); excl of the last batch = total - n_iter(last)
-            unsigned last_ni = 0;
-            for (int q = 0; q < 16; ++q) last_ni = max(last_ni, max(unit_count(q, 2 * (NB - 1)), unit_count(q, 2 * (NB - 1) + 1)));
-            totals[band].items = (total_iters - last_ni) / ITEM_ITERS + 1;
+            totals[band].items = (total_iters - batch_iters(NB - 1)) / ITEM_ITERS + 1;
         }
         return;
-    }
+    } else {
     // ---------------- PASS 2: lane words (idle default first), then every thread emits its cell's units
     for (unsigned i = t; i < NB * 32; i += XCELLS) { blane[(size_t)nb0 * 32 + i] = 0; lsrc[(size_t)nb0 * 32 + i] = 0; }
     __syncthreads();
     auto emit = [&](unsigned g, unsigned count, unsigned src) {
-        const unsigned b = g >> 1, lane = (g & 1) * 16 + r;
-        blane[(size_t)(nb0 + b) * 32 + lane] = (unsigned)cell | (count << 16);
-        lsrc[(size_t)(nb0 + b) * 32 + lane] = src;
+        blane[(size_t)nb0 * 32 + g] = (unsigned)t | (count << 16);
+        lsrc[(size_t)nb0 * 32 + g] = src;
     };
-    // full units in layer-major order: unit (m, j) at  g = sum_q min(full_q, j) + #{q < m : full_q > j}
-    {
-        unsigned G = 0;                                   // sum_q min(full_q, j)
-        for (unsigned j = 0; j < myfull; ++j) {
-            unsigned Nj = 0, pos = 0, lastq = 0;
-            for (int q = 0; q < 32; ++q) {
-                const bool in = s_full[r][q] > j;
-                Nj += in; if (in && q < m) ++pos; if (in) lastq = q;
-            }
-            const unsigned g = G + pos;
-            emit(g, UNIT_CAP, s_start[r][m] + j * UNIT_CAP);
-            // duplicate-cell check: odd g whose predecessor (g - 1) is the same cell
-            if ((g & 1) && pos == 0 && j > 0) {
-                unsigned lastprev = 0;
-                for (int q = 0; q < 32; ++q) if (s_full[r][q] > j - 1) lastprev = q;
-                if (lastprev == (unsigned)m) atomicOr(&bhdr[nb0 + (g >> 1)].y, 1u << 16);
-            }
-            (void)lastq;
-            G += Nj;
+    // full units, layer by layer: layer j holds the cells with more than j full units, cells ascending
+    unsigned G = 0;                                       // units before layer j
+    for (unsigned j = 0; j < maxfull; ++j) {
+        const bool in = myfull > j;
+        const unsigned bal = __ballot_sync(0xffffffffu, in);
+        if (lane == 0) s_w[warp] = __popc(bal);
+        __syncthreads();
+        unsigned pre = 0, N = 0;
+        for (int q = 0; q < XCELLS / 32; ++q) { const unsigned c = s_w[q]; if (q < warp) pre += c; N += c; }
+        if (in) {
+            const unsigned g = G + pre + __popc(bal & ((1u << lane) - 1u));
+            emit(g, UNIT_CAP, start + j * UNIT_CAP);
+            // the batch leaves this layer => it may hold one cell twice
+            const unsigned b0 = g & ~31u;
+            if (b0 < G || min(b0 + 32u, Q) > G + N) atomicOr(&bhdr[nb0 + (g >> 5)].y, 1u << 16);
         }
+        G += N;
+        __syncthreads();
     }
-    if (myrem > 0) {
-        const unsigned g = s_F[r] + rank;
-        emit(g, myrem, s_start[r][m] + myfull * UNIT_CAP);
-        if ((g & 1) && rank == 0 && myfull > 0) {
-            unsigned lastprev = 0;
-            for (int q = 0; q < 32; ++q) if (s_full[r][q] > s_maxfull[r] - 1) lastprev = q;
-            if (lastprev == (unsigned)m && myfull == s_maxfull[r]) atomicOr(&bhdr[nb0 + (g >> 1)].y, 1u << 16);
+    if (myrem) {
+        const unsigned g = F + rank;
+        emit(g, myrem, start + myfull * UNIT_CAP);
+        if ((g & ~31u) < F) atomicOr(&bhdr[nb0 + (g >> 5)].y, 1u << 16);
+    }
+    // ---- bank-aware lane assignment.  Which lane of a batch runs which unit is free; the 16 lanes of
+    // a half-warp access the box together with 8-byte words, and two of them collide when their
+    // cells fall into the same class (ly * boxw + lx) mod 16.  Sort the batch's units by class and
+    // deal them alternately to the two half-warps, so that the cells of one class are split evenly.
+    __syncthreads();
+    for (unsigned b = warp; b < NB; b += XCELLS / 32) {
+        const size_t o = (size_t)(nb0 + b) * 32 + lane;
+        const unsigned lw = blane[o], src = lsrc[o];
+        const unsigned cell = lw & 0x1FFu;
+        const unsigned key = (lw >> 16) == 0 ? 16u : (((cell >> 5) * (unsigned)boxw + (cell & 31u)) & 15u);   // idle lanes last
+        unsigned r = 0;
+        for (int q = 0; q < 32; ++q) {
+            const unsigned kq = __shfl_sync(0xffffffffu, key, q);
+            r += (kq < key || (kq == key && q < lane)) ? 1u : 0u;
         }
+        const unsigned dstl = (r & 1u) * 16u + (r >> 1);
+        __syncwarp();
+        blane[(size_t)(nb0 + b) * 32 + dstl] = lw;
+        lsrc[(size_t)(nb0 + b) * 32 + dstl] = src;
+    }
     }
 }
 
@@ -290,12 +280,12 @@ __global__ void split_totals_kernel(const BandTotals* __restrict__ t, int n_band
     if (t[i].nb) atomicAdd(nonempty, 1u);
 }
 
-// a0.4: fill the slots of every batch (one warp per batch): permutation, reduced (u, v), weights.
+// a0.4: fill the slots of every batch (one warp per batch): permutation and the per-iteration
+// records (reduced (u, v), weights).
 __global__ void __launch_bounds__(256)
 slot_fill_kernel(const uint2* __restrict__ bhdr, const unsigned* __restrict__ blane, const unsigned* __restrict__ lsrc,
                  unsigned n_batches, const unsigned* __restrict__ perm0, const float2* __restrict__ uv,
-                 const float* __restrict__ w, int K,
-                 unsigned* __restrict__ perm, float2* __restrict__ uv_s, float* __restrict__ w_s) {
+                 const float* __restrict__ w, int K, unsigned* __restrict__ perm, float* __restrict__ rec) {
     const unsigned warps = (gridDim.x * blockDim.x) >> 5;
     const int lane = threadIdx.x & 31;
     for (unsigned b = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; b < n_batches; b += warps) {
@@ -309,20 +299,30 @@ slot_fill_kernel(const uint2* __restrict__ bhdr, const unsigned* __restrict__ bl
             pad = make_float2(x_reduce(c.x, K), x_reduce(c.y, K));
         }
         for (unsigned i = 0; i < n_iter; ++i) {
-            const size_t slot = ((size_t)h.x + i) * 32 + lane;
+            const size_t it = (size_t)h.x + i;
+            float* r = rec + it * REC_FLOATS;
+            float2 c = pad;
+            float wv = 0.f;
+            unsigned pi = PERM_PAD;
             if (i < cnt) {
-                const unsigned p = perm0[src + i];
-                const float2 c = uv[p];
-                perm[slot] = p;
-                uv_s[slot] = make_float2(x_reduce(c.x, K), x_reduce(c.y, K));
-                w_s[slot] = w ? w[p] : 1.f;
-            } else {
-                perm[slot] = PERM_PAD;
-                uv_s[slot] = pad;
-                w_s[slot] = 0.f;
+                pi = perm0[src + i];
+                const float2 c0 = uv[pi];
+                c = make_float2(x_reduce(c0.x, K), x_reduce(c0.y, K));
+                wv = w ? w[pi] : 1.f;
             }
+            perm[it * 32 + lane] = pi;
+            reinterpret_cast<float2*>(r)[lane] = c;
+            r[64 + lane] = wv;
         }
     }
+}
+
+// a0.5: iteration count of every item (its slots are one contiguous stream of `iters` x 32 slots).
+__global__ void item_iters_kernel(XItem* __restrict__ items, int n_items, const uint2* __restrict__ bhdr) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_items) return;
+    const uint2 h = bhdr[items[i].end - 1];
+    items[i].iters = h.x + (h.y & 0xFFFFu) - items[i].iter0;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -370,18 +370,10 @@ __device__ __forceinline__ unsigned x_next_item(unsigned* counter, int lane) {
     return __shfl_sync(0xffffffffu, it, 0);
 }
 
-// a0.5: iteration count of every item (its slots are one contiguous stream of `iters` x 32 slots).
-__global__ void item_iters_kernel(XItem* __restrict__ items, int n_items, const uint2* __restrict__ bhdr) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n_items) return;
-    const uint2 h = bhdr[items[i].end - 1];
-    items[i].iters = h.x + (h.y & 0xFFFFu) - items[i].iter0;
-}
-
 // ---------------------------------------------------------------------------------------------
 // Visibility stream ring.  The slots of one item are contiguous in HBM, so every warp streams them
 // through a private ring of S stages in shared memory, each filled by 1-D bulk copies
-// (cp.async.bulk, mbarrier completion) of CH iterations (CH x 32 slots): uv, w and - for the
+// (cp.async.bulk, mbarrier completion) of CH iterations: the records (uv, w) and - for the
 // adjoint - y.  The copies run S-1 chunks ahead of the arithmetic, which is what hides the HBM
 // latency (profiles/r1b_summary.md: with a one-deep register prefetch both kernels were
 // long-scoreboard bound at 32 % issue utilisation).
@@ -391,29 +383,29 @@ __device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gsrc, uint3
 }
 
 template <int CH, bool WITH_Y> struct RingCfg {
-    static constexpr int UV = CH * 256, W = CH * 128, Y = WITH_Y ? CH * 256 : 0;
-    static constexpr int STAGE = UV + W + Y;
+    static constexpr int REC = CH * REC_BYTES, Y = WITH_Y ? CH * 256 : 0;
+    static constexpr int STAGE = REC + Y;
 };
 
 template <int J, int CH, int S, bool WITH_Y> struct XSmem {
     static constexpr int WARP_BYTES = XCfg<J>::REGION_BYTES + S * RingCfg<CH, WITH_Y>::STAGE;
-    static constexpr int BARS = S + 1;                   // per warp: ring stages + the box
+    static constexpr int BARS = S + 1;                   // per warp: the box + the ring stages
     static constexpr size_t TOTAL = (size_t)XCfg<J>::WARPS * WARP_BYTES + XCfg<J>::WARPS * BARS * sizeof(uint64_t);
 };
 
-// lane 0: start the copies of chunk c (iterations [c CH, c CH + n)) of the item into `stage`
+// one lane: start the copies of chunk c (iterations [c CH, c CH + n)) of the item into `stage`.
+// (No proxy fence: the stage was only READ through the generic proxy, and those reads are ordered
+// before this call by the __syncwarp() that precedes it.)
 template <int CH, bool WITH_Y>
 __device__ __forceinline__ void ring_issue(unsigned char* ring, uint64_t* rbar, int stage, const XParams& p,
                                            const float2* y, unsigned iter0, int c, int T) {
     typedef RingCfg<CH, WITH_Y> R;
     const int n = min(CH, T - c * CH);
-    const size_t s0 = ((size_t)iter0 + (size_t)c * CH) * 32;
+    const size_t i0 = (size_t)iter0 + (size_t)c * CH;
     unsigned char* st = ring + stage * R::STAGE;
-    fence_proxy_async();
-    mbar_expect_tx(rbar + stage, (uint32_t)(n * (256 + 128 + (WITH_Y ? 256 : 0))));
-    bulk_g2s(st, p.uv + s0, (uint32_t)(n * 256), rbar + stage);
-    bulk_g2s(st + R::UV, p.w + s0, (uint32_t)(n * 128), rbar + stage);
-    if (WITH_Y) bulk_g2s(st + R::UV + R::W, y + s0, (uint32_t)(n * 256), rbar + stage);
+    mbar_expect_tx(rbar + stage, (uint32_t)(n * (REC_BYTES + (WITH_Y ? 256 : 0))));
+    bulk_g2s(st, p.rec + i0 * REC_FLOATS, (uint32_t)(n * REC_BYTES), rbar + stage);
+    if (WITH_Y) bulk_g2s(st + R::REC, y + i0 * 32, (uint32_t)(n * 256), rbar + stage);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -442,8 +434,15 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
     uint32_t box_phase = 0, ring_phase = 0;
     int stage = 0;
 
-    for (unsigned item = x_next_item(p.counter, lane); item < (unsigned)p.n_items; item = x_next_item(p.counter, lane)) {
-        const XItem it = p.items[item];
+    // the NEXT item (index and descriptor) is fetched while the current one is processed
+    unsigned item = x_next_item(p.counter, lane);
+    XItem nit = p.items[min(item, (unsigned)p.n_items - 1)];
+    uint2 hn = p.bhdr[nit.begin];
+    unsigned lwn = p.blane[(size_t)nit.begin * 32 + lane];
+    while (item < (unsigned)p.n_items) {
+        const XItem it = nit;
+        item = x_next_item(p.counter, lane);
+        nit = p.items[min(item, (unsigned)p.n_items - 1)];
         const int T = (int)it.iters, nch = (T + CH - 1) / CH;
         const int bx0 = it.x0 - (J / 2 - 1) - XOFF, by0 = it.y0 - (J / 2 - 1);
         const bool interior = bx0 >= 0 && by0 >= 0 && bx0 + BOXW <= p.K && by0 + BOXH <= p.K;
@@ -460,8 +459,7 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
                 st = st + 1 == S ? 0 : st + 1;
             }
         }
-        uint2 hn = p.bhdr[it.begin];
-        unsigned lwn = p.blane[(size_t)it.begin * 32 + lane];
+        int cnext = S;                                  // next chunk to start
         if (interior) {
             mbar_wait(bar, box_phase);
             box_phase ^= 1;
@@ -472,12 +470,18 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
             }
             __syncwarp();
         }
-        int gi = 0;                                     // iteration within the item
+        int left = T;                                   // iterations of the item not yet started
+        int rem = 0;                                    // iterations left in the current chunk
+        const float* rp = nullptr;                      // this lane's view of the current record
         float2* yout = y + (size_t)it.iter0 * 32 + lane;
         for (int b = it.begin; b < it.end; ++b) {
             const uint2 h = hn;
             const unsigned lw = lwn;
-            if (b + 1 < it.end) { hn = p.bhdr[b + 1]; lwn = p.blane[(size_t)(b + 1) * 32 + lane]; }
+            {                                           // header of the next batch (of this or of the next item)
+                const int bn = b + 1 < it.end ? b + 1 : nit.begin;
+                hn = p.bhdr[bn];
+                lwn = p.blane[(size_t)bn * 32 + lane];
+            }
             const int n_iter = (int)(h.y & 0xFFFFu);
             const int ly = (lw >> 5) & 15, lx = lw & 31;
             const int cx = it.x0 + lx - p.Kh, cy = it.y0 + ly - p.Kh;       // cell = floor(u'), floor(v')
@@ -490,12 +494,16 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
 #pragma unroll
                     for (int c = 0; c < J; ++c) B[a][c] = src[a * BOXW + c];
             }
-            for (int i = 0; i < n_iter; ++i, ++gi) {
-                const int off = gi & (CH - 1);
-                if (off == 0) mbar_wait(rbar + stage, ring_phase);
-                const unsigned char* st = ring + stage * R::STAGE;
-                const float2 uvk = reinterpret_cast<const float2*>(st)[off * 32 + lane];
-                const float wk = reinterpret_cast<const float*>(st + R::UV)[off * 32 + lane];
+            for (int i = 0; i < n_iter; ++i) {
+                if (rem == 0) {
+                    mbar_wait(rbar + stage, ring_phase);
+                    rem = min(CH, left);
+                    left -= rem;
+                    rp = reinterpret_cast<const float*>(ring + stage * R::STAGE) + lane;
+                }
+                const float2 uvk = *reinterpret_cast<const float2*>(rp + lane);
+                const float wk = rp[64];
+                rp += REC_FLOATS;
                 float2 g[J];
                 x_weights<J, DEG, MODE>(uvk, cellf, cx, cy, p, g);
                 float2 acc = make_float2(0.f, 0.f);
@@ -506,11 +514,14 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
                     for (int c = 1; c < J; ++c) row = fma2(dup2(g[c].x), B[a][c], row);
                     acc = fma2(dup2(g[a].y), row, acc);
                 }
-                yout[(size_t)gi * 32] = mul2(dup2(wk), acc);                // padding slots: w = 0 -> 0
-                if (off == CH - 1 || gi == T - 1) {                         // chunk consumed: refill its stage
+                *yout = mul2(dup2(wk), acc);                                // padding slots: w = 0 -> 0
+                yout += 32;
+                if (--rem == 0) {                                           // chunk consumed: refill its stage
                     __syncwarp();
-                    const int cn = gi / CH + S;
-                    if (lane == 0 && cn < nch) ring_issue<CH, false>(ring, rbar, stage, p, nullptr, it.iter0, cn, T);
+                    if (cnext < nch) {
+                        if (lane == 0) ring_issue<CH, false>(ring, rbar, stage, p, nullptr, it.iter0, cnext, T);
+                        ++cnext;
+                    }
                     if (++stage == S) { stage = 0; ring_phase ^= 1; }
                 }
             }
@@ -521,11 +532,12 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
 // ---------------------------------------------------------------------------------------------
 // a4 (complex64): G^dagger W^dagger.  Same items / batches / ring (with y).  Every lane accumulates
 // its unit's J x J outer products in registers; at the end of the batch the accumulators are added
-// into the warp's private shared-memory box (lanes of one pass hold distinct cells => distinct
-// addresses in every step, no atomics; __syncwarp orders the steps because footprints of different
-// lanes overlap); at the end of the item the box is added to the global grid with one 8-byte
-// reduction per non-zero cell (RED.ADD.F32x2; halos of neighbouring bands and the items of one band
-// meet there).
+// into the warp's private shared-memory box: lanes of an unflagged batch hold distinct cells =>
+// distinct addresses in every step, plain read-modify-writes (__syncwarp orders the steps because
+// footprints of different lanes overlap); a flagged batch (a cell may occur twice) uses
+// shared-memory atomics.  At the end of the item the box is added to the global grid with one
+// 8-byte reduction per non-zero cell (RED.ADD.F32x2; halos of neighbouring bands and the items of
+// one band meet there).
 template <int J, int DEG, int MODE, int CH, int S>
 __global__ void __launch_bounds__(XCfg<J>::THREADS)
 grid_x_kernel(const XParams p, const float2* __restrict__ y) {
@@ -547,8 +559,14 @@ grid_x_kernel(const XParams p, const float2* __restrict__ y) {
     uint32_t ring_phase = 0;
     int stage = 0;
 
-    for (unsigned item = x_next_item(p.counter, lane); item < (unsigned)p.n_items; item = x_next_item(p.counter, lane)) {
-        const XItem it = p.items[item];
+    unsigned item = x_next_item(p.counter, lane);
+    XItem nit = p.items[min(item, (unsigned)p.n_items - 1)];
+    uint2 hn = p.bhdr[nit.begin];
+    unsigned lwn = p.blane[(size_t)nit.begin * 32 + lane];
+    while (item < (unsigned)p.n_items) {
+        const XItem it = nit;
+        item = x_next_item(p.counter, lane);
+        nit = p.items[min(item, (unsigned)p.n_items - 1)];
         const int T = (int)it.iters, nch = (T + CH - 1) / CH;
         if (lane == 0) {
             int st = stage;
@@ -557,17 +575,22 @@ grid_x_kernel(const XParams p, const float2* __restrict__ y) {
                 st = st + 1 == S ? 0 : st + 1;
             }
         }
-        uint2 hn = p.bhdr[it.begin];
-        unsigned lwn = p.blane[(size_t)it.begin * 32 + lane];
+        int cnext = S;
         for (int i = lane; i < BOXW * BOXH; i += 32) tile[i] = make_float2(0.f, 0.f);
         __syncwarp();
-        int gi = 0;
+        int left = T, rem = 0;
+        const float* rp = nullptr;
+        const float2* yp = nullptr;
         for (int b = it.begin; b < it.end; ++b) {
             const uint2 h = hn;
             const unsigned lw = lwn;
-            if (b + 1 < it.end) { hn = p.bhdr[b + 1]; lwn = p.blane[(size_t)(b + 1) * 32 + lane]; }
+            {
+                const int bn = b + 1 < it.end ? b + 1 : nit.begin;
+                hn = p.bhdr[bn];
+                lwn = p.blane[(size_t)bn * 32 + lane];
+            }
             const int n_iter = (int)(h.y & 0xFFFFu);
-            const bool two_pass = (h.y >> 16) & 1u;
+            const bool dup = (h.y >> 16) & 1u;
             const int cnt = (int)(lw >> 16);
             const int ly = (lw >> 5) & 15, lx = lw & 31;
             const int cx = it.x0 + lx - p.Kh, cy = it.y0 + ly - p.Kh;
@@ -578,13 +601,19 @@ grid_x_kernel(const XParams p, const float2* __restrict__ y) {
 #pragma unroll
                 for (int c = 0; c < J; ++c) A[a][c] = make_float2(0.f, 0.f);
 
-            for (int i = 0; i < n_iter; ++i, ++gi) {
-                const int off = gi & (CH - 1);
-                if (off == 0) mbar_wait(rbar + stage, ring_phase);
-                const unsigned char* st = ring + stage * R::STAGE;
-                const float2 uvk = reinterpret_cast<const float2*>(st)[off * 32 + lane];
-                const float wk = reinterpret_cast<const float*>(st + R::UV)[off * 32 + lane];
-                float2 yk = reinterpret_cast<const float2*>(st + R::UV + R::W)[off * 32 + lane];
+            for (int i = 0; i < n_iter; ++i) {
+                if (rem == 0) {
+                    mbar_wait(rbar + stage, ring_phase);
+                    rem = min(CH, left);
+                    left -= rem;
+                    rp = reinterpret_cast<const float*>(ring + stage * R::STAGE) + lane;
+                    yp = reinterpret_cast<const float2*>(ring + stage * R::STAGE + R::REC) + lane;
+                }
+                const float2 uvk = *reinterpret_cast<const float2*>(rp + lane);
+                const float wk = rp[64];
+                float2 yk = *yp;
+                rp += REC_FLOATS;
+                yp += 32;
                 if (i >= cnt) yk = make_float2(0.f, 0.f);                   // padding slot: whatever y holds there is ignored
                 float2 g[J];
                 x_weights<J, DEG, MODE>(uvk, cellf, cx, cy, p, g);
@@ -595,26 +624,36 @@ grid_x_kernel(const XParams p, const float2* __restrict__ y) {
 #pragma unroll
                     for (int c = 0; c < J; ++c) A[a][c] = fma2(dup2(g[c].x), q, A[a][c]);
                 }
-                if (off == CH - 1 || gi == T - 1) {
+                if (--rem == 0) {
                     __syncwarp();
-                    const int cn = gi / CH + S;
-                    if (lane == 0 && cn < nch) ring_issue<CH, true>(ring, rbar, stage, p, y, it.iter0, cn, T);
+                    if (cnext < nch) {
+                        if (lane == 0) ring_issue<CH, true>(ring, rbar, stage, p, y, it.iter0, cnext, T);
+                        ++cnext;
+                    }
                     if (++stage == S) { stage = 0; ring_phase ^= 1; }
                 }
             }
-            // ---- flush the accumulators into the warp's box.  Idle lanes (no unit) stay out; a batch
-            // that holds one cell twice (lanes r and 16 + r) flushes its two half-warps one after the other.
+            // ---- flush the accumulators into the warp's box; idle lanes (no unit) stay out
             float2* dst = tile + ly * BOXW + lx + XOFF;
-            const int n_pass = two_pass ? 2 : 1;
-            for (int pass = 0; pass < n_pass; ++pass) {
-                const bool act = cnt > 0 && (!two_pass || (lane >> 4) == pass);
+            if (!dup) {
 #pragma unroll
                 for (int a = 0; a < J; ++a)
 #pragma unroll
                     for (int c = 0; c < J; ++c) {
-                        if (act) dst[a * BOXW + c] = add2(dst[a * BOXW + c], A[a][c]);
+                        if (cnt > 0) dst[a * BOXW + c] = add2(dst[a * BOXW + c], A[a][c]);
                         __syncwarp();
                     }
+            } else {
+                if (cnt > 0) {
+#pragma unroll
+                    for (int a = 0; a < J; ++a)
+#pragma unroll
+                        for (int c = 0; c < J; ++c) {
+                            atomicAdd(&dst[a * BOXW + c].x, A[a][c].x);
+                            atomicAdd(&dst[a * BOXW + c].y, A[a][c].y);
+                        }
+                }
+                __syncwarp();
             }
         }
         // ---- add the box to the global grid (periodic wrap here)

@@ -197,9 +197,8 @@ pk::XParams make_xparams(const purify_op* op, bool caller_order) {
     p.counter = op->x_counter;
     p.bhdr = op->x_bhdr;
     p.blane = op->x_blane;
-    p.uv = (const float2*)op->uv_s;
-    p.w = (const float*)op->w_s;
-    p.perm = caller_order ? op->perm : nullptr;
+    p.rec = (const float*)op->uv_s;
+    (void)caller_order;
     memcpy(&p.coef, &op->coef32, sizeof(p.coef));
     p.table = (const float*)op->table;
     p.table_R = (float)op->table_R;
@@ -224,21 +223,28 @@ template <typename Kern> int x_grid_size(Kern kern, int threads, size_t smem, in
 }
 
 // ring geometry of the complex64 kernels: CH iterations per chunk, S stages (batched.cuh "ring")
-constexpr int X_CH = 4, X_S_DEGRID = 4, X_S_GRID = 3;
+// ring geometry (chunk iterations, stages) of the two complex64 kernels; -D overrides are for tuning builds
+#ifndef PURIFY_X_CHD
+#define PURIFY_X_CHD 8
+#define PURIFY_X_SD 2
+#define PURIFY_X_CHG 6
+#define PURIFY_X_SG 2
+#endif
+constexpr int X_CH_DEGRID = PURIFY_X_CHD, X_S_DEGRID = PURIFY_X_SD, X_CH_GRID = PURIFY_X_CHG, X_S_GRID = PURIFY_X_SG;
 
 template <int J, int DEG> int launch_degrid_x_t(purify_op* op, void* y, cudaStream_t st) {
     typedef pk::XCfg<J> Cfg;
     if (op->n_items == 0) return PURIFY_OK;
-    const size_t smem = pk::XSmem<J, X_CH, X_S_DEGRID, false>::TOTAL;
+    const size_t smem = pk::XSmem<J, X_CH_DEGRID, X_S_DEGRID, false>::TOTAL;
     const pk::XParams p = make_xparams(op, false);
     CK(cudaMemsetAsync(op->x_counter, 0, sizeof(unsigned), st));
     int g = 0, rc;
     if (op->mode == PURIFY_KERNEL_TABLE) {
-        auto kern = pk::degrid_x_kernel<J, DEG, 1, X_CH, X_S_DEGRID>;
+        auto kern = pk::degrid_x_kernel<J, DEG, 1, X_CH_DEGRID, X_S_DEGRID>;
         if ((rc = x_grid_size(kern, Cfg::THREADS, smem, op->n_items, Cfg::WARPS, &g))) return rc;
         kern<<<g, Cfg::THREADS, smem, st>>>(op->tmap_x, p, (float2*)y);
     } else {
-        auto kern = pk::degrid_x_kernel<J, DEG, 0, X_CH, X_S_DEGRID>;
+        auto kern = pk::degrid_x_kernel<J, DEG, 0, X_CH_DEGRID, X_S_DEGRID>;
         if ((rc = x_grid_size(kern, Cfg::THREADS, smem, op->n_items, Cfg::WARPS, &g))) return rc;
         kern<<<g, Cfg::THREADS, smem, st>>>(op->tmap_x, p, (float2*)y);
     }
@@ -250,16 +256,16 @@ template <int J, int DEG> int launch_degrid_x_t(purify_op* op, void* y, cudaStre
 template <int J, int DEG> int launch_grid_x_t(purify_op* op, const void* y, cudaStream_t st) {
     typedef pk::XCfg<J> Cfg;
     if (op->n_items == 0) return PURIFY_OK;
-    const size_t smem = pk::XSmem<J, X_CH, X_S_GRID, true>::TOTAL;
+    const size_t smem = pk::XSmem<J, X_CH_GRID, X_S_GRID, true>::TOTAL;
     const pk::XParams p = make_xparams(op, false);
     CK(cudaMemsetAsync(op->x_counter, 0, sizeof(unsigned), st));
     int g = 0, rc;
     if (op->mode == PURIFY_KERNEL_TABLE) {
-        auto kern = pk::grid_x_kernel<J, DEG, 1, X_CH, X_S_GRID>;
+        auto kern = pk::grid_x_kernel<J, DEG, 1, X_CH_GRID, X_S_GRID>;
         if ((rc = x_grid_size(kern, Cfg::THREADS, smem, op->n_items, Cfg::WARPS, &g))) return rc;
         kern<<<g, Cfg::THREADS, smem, st>>>(p, (const float2*)y);
     } else {
-        auto kern = pk::grid_x_kernel<J, DEG, 0, X_CH, X_S_GRID>;
+        auto kern = pk::grid_x_kernel<J, DEG, 0, X_CH_GRID, X_S_GRID>;
         if ((rc = x_grid_size(kern, Cfg::THREADS, smem, op->n_items, Cfg::WARPS, &g))) return rc;
         kern<<<g, Cfg::THREADS, smem, st>>>(p, (const float2*)y);
     }
@@ -511,7 +517,6 @@ int build_bins_x(purify_op* op, const void* uv_dev, const void* w_dev, cudaStrea
     const int K = op->K;
     const int nbx = (K + pk::XBW - 1) / pk::XBW, nby = (K + pk::XBH - 1) / pk::XBH;
     const int n_bands = nbx * nby;
-    const int boxw = pk::XBW + op->J;
     op->n_bands = n_bands;
     op->ntx = nbx;
     op->n_tiles = n_bands;
@@ -575,7 +580,7 @@ int build_bins_x(purify_op* op, const void* uv_dev, const void* w_dev, cudaStrea
     }
     pk::band_start_kernel<<<(n_bands + 1 + 255) / 256, 256, 0, st>>>(keys2, M, n_bands, band_start);
     CKC(cudaGetLastError());
-    pk::band_build_kernel<1><<<n_bands, pk::XCELLS, 0, st>>>(keys2, band_start, nbx, boxw, totals, nullptr, nullptr, nullptr,
+    pk::band_build_kernel<1><<<n_bands, pk::XCELLS, 0, st>>>(keys2, band_start, nbx, pk::XBW + op->J, totals, nullptr, nullptr, nullptr,
                                                              nullptr, nullptr, nullptr, nullptr);
     CKC(cudaGetLastError());
     pk::split_totals_kernel<<<(n_bands + 1 + 255) / 256, 256, 0, st>>>(totals, n_bands, a_nb, a_it, a_items, nonempty);
@@ -601,8 +606,8 @@ int build_bins_x(purify_op* op, const void* uv_dev, const void* w_dev, cudaStrea
     op->n_tiles_nonempty = (int)h_tot[3];
     int rc;
     const size_t S = op->M_native > 0 ? (size_t)op->M_native : 1, NBz = op->n_batches > 0 ? op->n_batches : 1;
-    if ((rc = dev_alloc(op, &op->uv_s, sizeof(float2) * S))) { cleanup(); return rc; }
-    if ((rc = dev_alloc(op, &op->w_s, sizeof(float) * S))) { cleanup(); return rc; }
+    // per-iteration records (uv[32] | w[32]); uv_s holds them, w_s is unused in this layout
+    if ((rc = dev_alloc(op, &op->uv_s, (size_t)pk::REC_BYTES * (S / 32 + 1)))) { cleanup(); return rc; }
     if ((rc = dev_alloc(op, (void**)&op->perm, sizeof(unsigned) * S))) { cleanup(); return rc; }
     if ((rc = dev_alloc(op, (void**)&op->x_bhdr, sizeof(uint2) * NBz))) { cleanup(); return rc; }
     if ((rc = dev_alloc(op, (void**)&op->x_blane, sizeof(unsigned) * 32 * NBz))) { cleanup(); return rc; }
@@ -610,14 +615,14 @@ int build_bins_x(purify_op* op, const void* uv_dev, const void* w_dev, cudaStrea
     if ((rc = dev_alloc(op, (void**)&op->x_counter, sizeof(unsigned)))) { cleanup(); return rc; }
     CKC(cudaMalloc(&lsrc, sizeof(unsigned) * 32 * NBz));
     if (op->n_batches > 0) {
-        pk::band_build_kernel<2><<<n_bands, pk::XCELLS, 0, st>>>(keys2, band_start, nbx, boxw, nullptr, o_nb, o_it, o_items,
+        pk::band_build_kernel<2><<<n_bands, pk::XCELLS, 0, st>>>(keys2, band_start, nbx, pk::XBW + op->J, nullptr, o_nb, o_it, o_items,
                                                                  op->x_bhdr, op->x_blane, lsrc, op->x_items);
         CKC(cudaGetLastError());
         pk::item_iters_kernel<<<(op->n_items + 255) / 256, 256, 0, st>>>(op->x_items, op->n_items, op->x_bhdr);
         CKC(cudaGetLastError());
         pk::slot_fill_kernel<<<grid_for((long long)op->n_batches * 32, 256), 256, 0, st>>>(
             op->x_bhdr, op->x_blane, lsrc, op->n_batches, perm0, (const float2*)uv_dev, (const float*)w_dev, K,
-            op->perm, (float2*)op->uv_s, (float*)op->w_s);
+            op->perm, (float*)op->uv_s);
         CKC(cudaGetLastError());
     }
     CKC(cudaStreamSynchronize(st));

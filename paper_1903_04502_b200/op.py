@@ -12,7 +12,7 @@ import os
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libpurify_op.so")
+LIB_PATH = os.environ.get("PURIFY_OP_LIB") or os.path.join(_HERE, "libpurify_op.so")   # env override: tuning builds
 
 C64, C128 = 0, 1
 ANALYTIC, TABLE = 0, 1
