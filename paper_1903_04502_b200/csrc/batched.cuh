@@ -494,29 +494,37 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
 #pragma unroll
                     for (int c = 0; c < J; ++c) B[a][c] = src[a * BOXW + c];
             }
-            for (int i = 0; i < n_iter; ++i) {
+            // the batch's iterations, cut into segments at the ring's chunk boundaries: the inner loop
+            // carries no ring logic
+            for (int i = 0; i < n_iter;) {
                 if (rem == 0) {
                     mbar_wait(rbar + stage, ring_phase);
                     rem = min(CH, left);
                     left -= rem;
                     rp = reinterpret_cast<const float*>(ring + stage * R::STAGE) + lane;
                 }
-                const float2 uvk = *reinterpret_cast<const float2*>(rp + lane);
-                const float wk = rp[64];
-                rp += REC_FLOATS;
-                float2 g[J];
-                x_weights<J, DEG, MODE>(uvk, cellf, cx, cy, p, g);
-                float2 acc = make_float2(0.f, 0.f);
+                const int seg = min(rem, n_iter - i);
+#pragma unroll 1
+                for (int k = 0; k < seg; ++k) {
+                    const float2 uvk = *reinterpret_cast<const float2*>(rp + lane);
+                    const float wk = rp[64];
+                    rp += REC_FLOATS;
+                    float2 g[J];
+                    x_weights<J, DEG, MODE>(uvk, cellf, cx, cy, p, g);
+                    float2 acc = make_float2(0.f, 0.f);
 #pragma unroll
-                for (int a = 0; a < J; ++a) {
-                    float2 row = mul2(dup2(g[0].x), B[a][0]);
+                    for (int a = 0; a < J; ++a) {
+                        float2 row = mul2(dup2(g[0].x), B[a][0]);
 #pragma unroll
-                    for (int c = 1; c < J; ++c) row = fma2(dup2(g[c].x), B[a][c], row);
-                    acc = fma2(dup2(g[a].y), row, acc);
+                        for (int c = 1; c < J; ++c) row = fma2(dup2(g[c].x), B[a][c], row);
+                        acc = fma2(dup2(g[a].y), row, acc);
+                    }
+                    *yout = mul2(dup2(wk), acc);                            // padding slots: w = 0 -> 0
+                    yout += 32;
                 }
-                *yout = mul2(dup2(wk), acc);                                // padding slots: w = 0 -> 0
-                yout += 32;
-                if (--rem == 0) {                                           // chunk consumed: refill its stage
+                i += seg;
+                rem -= seg;
+                if (rem == 0) {                                             // chunk consumed: refill its stage
                     __syncwarp();
                     if (cnext < nch) {
                         if (lane == 0) ring_issue<CH, false>(ring, rbar, stage, p, nullptr, it.iter0, cnext, T);
@@ -601,7 +609,7 @@ grid_x_kernel(const XParams p, const float2* __restrict__ y) {
 #pragma unroll
                 for (int c = 0; c < J; ++c) A[a][c] = make_float2(0.f, 0.f);
 
-            for (int i = 0; i < n_iter; ++i) {
+            for (int i = 0; i < n_iter;) {
                 if (rem == 0) {
                     mbar_wait(rbar + stage, ring_phase);
                     rem = min(CH, left);
@@ -609,22 +617,29 @@ grid_x_kernel(const XParams p, const float2* __restrict__ y) {
                     rp = reinterpret_cast<const float*>(ring + stage * R::STAGE) + lane;
                     yp = reinterpret_cast<const float2*>(ring + stage * R::STAGE + R::REC) + lane;
                 }
-                const float2 uvk = *reinterpret_cast<const float2*>(rp + lane);
-                const float wk = rp[64];
-                float2 yk = *yp;
-                rp += REC_FLOATS;
-                yp += 32;
-                if (i >= cnt) yk = make_float2(0.f, 0.f);                   // padding slot: whatever y holds there is ignored
-                float2 g[J];
-                x_weights<J, DEG, MODE>(uvk, cellf, cx, cy, p, g);
-                const float2 z = mul2(dup2(wk), yk);
+                const int seg = min(rem, n_iter - i);
+                int live = cnt - i;                                         // slots of this segment that hold a visibility
+#pragma unroll 1
+                for (int k = 0; k < seg; ++k, --live) {
+                    const float2 uvk = *reinterpret_cast<const float2*>(rp + lane);
+                    const float wk = rp[64];
+                    float2 yk = *yp;
+                    rp += REC_FLOATS;
+                    yp += 32;
+                    if (live <= 0) yk = make_float2(0.f, 0.f);              // padding slot: whatever y holds there is ignored
+                    float2 g[J];
+                    x_weights<J, DEG, MODE>(uvk, cellf, cx, cy, p, g);
+                    const float2 z = mul2(dup2(wk), yk);
 #pragma unroll
-                for (int a = 0; a < J; ++a) {
-                    const float2 q = mul2(dup2(g[a].y), z);
+                    for (int a = 0; a < J; ++a) {
+                        const float2 q = mul2(dup2(g[a].y), z);
 #pragma unroll
-                    for (int c = 0; c < J; ++c) A[a][c] = fma2(dup2(g[c].x), q, A[a][c]);
+                        for (int c = 0; c < J; ++c) A[a][c] = fma2(dup2(g[c].x), q, A[a][c]);
+                    }
                 }
-                if (--rem == 0) {
+                i += seg;
+                rem -= seg;
+                if (rem == 0) {
                     __syncwarp();
                     if (cnext < nch) {
                         if (lane == 0) ring_issue<CH, true>(ring, rbar, stage, p, y, it.iter0, cnext, T);
