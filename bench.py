@@ -189,10 +189,9 @@ def run_ours(args):
     import torch.distributed as dist
 
     from paper_1903_04502_b200 import ANALYTIC, C64, C128, TABLE, PurifyOp, synth
+    from paper_1903_04502_b200 import dist as pdist
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, local_rank, world = pdist.world()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference for the oracle)")
     torch.cuda.set_device(local_rank)
@@ -205,8 +204,7 @@ def run_ours(args):
     cbytes = 8 if cfg.dtype == "c64" else 16
     rbytes = cbytes // 2
     # every rank draws its OWN visibility set (weak scaling): seed offset by rank
-    import dataclasses
-    rcfg = dataclasses.replace(cfg, index=cfg.index + 100 * rank) if rank else cfg
+    rcfg = pdist.rank_config(cfg, rank)
     t_gen = time.perf_counter()
     x = synth.make_image(cfg.n, cfg.seed, cfg.dtype)
     uv = synth.make_uv(rcfg, M)
@@ -228,8 +226,7 @@ def run_ours(args):
 
     def step():
         op.normal(x_dev, out_dev)
-        if world > 1:
-            dist.all_reduce(torch.view_as_real(out_dev))        # Eq. (38): sum of the per-rank dirty images
+        pdist.allreduce_image(out_dev)                          # Eq. (38): sum of the per-rank dirty images
 
     def barrier():
         if world > 1:
@@ -251,10 +248,7 @@ def run_ours(args):
     barrier()
     ms_total = e0.elapsed_time(e1)
     launches = op.last_launch_count() * args.steps
-    if world > 1:
-        tt = torch.tensor([ms_total], device="cuda")
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms_total = float(tt.item())
+    ms_total = pdist.max_over_ranks(ms_total, device="cuda")
     ms_step = ms_total / args.steps
 
     # ---- per-stage breakdown (separate pass; each step followed by a sync to read the stage events)
@@ -297,10 +291,7 @@ def run_ours(args):
             pass    # the host-buffer path is single-GPU; the image all-reduce is in the device arm
     torch.cuda.synchronize()
     e2e_s = (time.perf_counter() - t0) / args.steps
-    if world > 1:
-        tt = torch.tensor([e2e_s], device="cuda")
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        e2e_s = float(tt.item())
+    e2e_s = pdist.max_over_ranks(e2e_s, device="cuda")
 
     if rank == 0:
         peak, peak_src = measured_peak()

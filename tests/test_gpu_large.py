@@ -1,0 +1,104 @@
+"""Parity at BASELINE.json's FULL sizes (configs 3, 4, 5), through the C ABI in the launch configuration
+bench.py times (native order, default options).  -m gpu
+
+The oracle is fast enough (OpenMP) to compute the whole Phi x and Phi^dagger y at these sizes, so the
+comparison is over the complete outputs, plus properties that hold at any size (adjoint identity,
+order invariance).  Tolerance: rel-L2 <= 1e-5 (complex64), <= 1e-12 (complex128) - BASELINE.json north_star.
+Set PURIFY_SKIP_HUGE=1 to skip config 5 (5e8 visibilities: ~50 GB of host memory, minutes of CPU oracle)."""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_1903_04502_b200 import synth
+
+pytestmark = [pytest.mark.gpu, pytest.mark.slow]
+
+TOL = {"c128": 1e-12, "c64": 1e-5}
+
+
+def rel_l2(a, b):
+    a = np.asarray(a).ravel()
+    b = np.asarray(b).ravel()
+    num = den = 0.0
+    step = 1 << 24                                    # blockwise: no M-sized complex128 temporaries
+    for i in range(0, len(b), step):
+        bb = b[i:i + step].astype(np.complex128)
+        d = a[i:i + step].astype(np.complex128) - bb
+        num += float(np.vdot(d, d).real)
+        den += float(np.vdot(bb, bb).real)
+    return (num / den) ** 0.5
+
+
+def full_size_checks(cfg, x, uv, w, dtype, order=None):
+    """Phi and Phi^dagger over the whole visibility set against the oracle; returns (y_gpu caller order, image)."""
+    from paper_1903_04502_b200 import ANALYTIC, C64, C128, TABLE, PurifyOp
+    cd, rd = synth.complex_dtype(dtype), synth.real_dtype(dtype)
+    x, uv, w = x.astype(cd), np.ascontiguousarray(uv.astype(rd)), w.astype(rd)
+    if order is not None:
+        uv, w = np.ascontiguousarray(uv[order]), np.ascontiguousarray(w[order])
+    M, tol = len(uv), TOL[dtype]
+    table = cfg.kernel_mode == "table"
+    okw = dict(mode=cfg.kernel_mode, R=cfg.table_R, idx_prec=32 if dtype == "c64" else 64)
+    op = PurifyOp(cfg.n, cfg.J, torch.from_numpy(uv).cuda(), torch.from_numpy(w).cuda(),
+                  dtype=C64 if dtype == "c64" else C128, kernel_mode=TABLE if table else ANALYTIC,
+                  table_samples_per_unit=cfg.table_R if table else 0)
+    info = op.info()
+    assert info["M"] == M and info["M_native"] >= M
+    xd = torch.from_numpy(x).cuda()
+    # ---- Phi, native order (what bench.py times), compared through the permutation
+    y_nat = op.degrid(xd, native=True)
+    y = op.permute_from_native(y_nat).cpu().numpy()
+    y_ref = oracle.degrid(x, uv, w, cfg.J, **okw)
+    assert rel_l2(y, y_ref) <= tol
+    y_call = op.degrid(xd).cpu().numpy()
+    assert np.array_equal(y_call, y)
+    # ---- Phi^dagger on the oracle's Phi x (rounded to storage), native order
+    yv = y_ref.astype(cd)
+    del y_ref
+    img_ref = oracle.grid(yv, uv, w, cfg.n, cfg.J, **okw)
+    yv_nat = op.permute_to_native(torch.from_numpy(yv).cuda())
+    img = op.grid(yv_nat, native=True).cpu().numpy()
+    assert rel_l2(img, img_ref) <= tol
+    # ---- Phi^dagger Phi (the bench step)
+    nrm = op.normal(xd).cpu().numpy()
+    assert rel_l2(nrm, img_ref) <= 3 * tol
+    # ---- adjoint identity with GPU results: <Phi x, y> = <x, Phi^dagger y>
+    lhs = complex(np.vdot(y.astype(np.complex128), yv.astype(np.complex128)))
+    rhs = complex(np.vdot(x.astype(np.complex128), img.astype(np.complex128)))
+    assert abs(lhs - rhs) / (np.linalg.norm(y.astype(np.complex128)) * np.linalg.norm(yv.astype(np.complex128))) <= 10 * tol
+    op.close()
+    del xd, y_nat, yv_nat
+    torch.cuda.empty_cache()
+    return y, img, info
+
+
+@pytest.mark.parametrize("dtype", ["c64", "c128"])
+def test_config3_rotation_synthesis_both_orders(dtype):
+    """BASELINE.json configs[2]: 1024^2 image, J=4, M=1e7 from a 27-antenna track; time-ordered and shuffled
+    input must give the same y up to the permutation (and the same image)."""
+    cfg, x, uv, w = synth.make_problem(3)
+    y_t, img_t, info = full_size_checks(cfg, x, uv, w, dtype)
+    order = synth.shuffle_order(cfg.M, cfg.seed)
+    y_s, img_s, _ = full_size_checks(cfg, x, uv, w, dtype, order=order)
+    assert np.array_equal(y_s, y_t[order])                       # each visibility is computed on its own: same bits
+    assert rel_l2(img_s, img_t) <= TOL[dtype]
+    if dtype == "c64":
+        assert info["layout"] == 1 and info["M_native"] < 1.5 * cfg.M
+
+
+def test_config4_full_size():
+    """BASELINE.json configs[3], the metric's config: 2048^2 image, J=6, M=1e8 Gaussian-density visibilities."""
+    cfg, x, uv, w = synth.make_problem(4)
+    _, _, info = full_size_checks(cfg, x, uv, w, "c64")
+    assert info["M_native"] <= 1.10 * cfg.M                      # padding of the batched layout stays small
+
+
+@pytest.mark.skipif(os.environ.get("PURIFY_SKIP_HUGE") == "1", reason="PURIFY_SKIP_HUGE=1")
+def test_config5_full_size_table_mode():
+    """BASELINE.json configs[4]: 4096^2 image, J=4, M=5e8 from a 197-antenna SKA-like layout, pre-sampled
+    kernel table with 4096 samples per unit."""
+    cfg, x, uv, w = synth.make_problem(5)
+    full_size_checks(cfg, x, uv, w, "c64")
