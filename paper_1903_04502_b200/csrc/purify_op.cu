@@ -231,16 +231,21 @@ template <typename Kern> int x_grid_size(Kern kern, int threads, size_t smem, in
 #define PURIFY_X_SG 2
 #endif
 constexpr int X_CH_DEGRID = PURIFY_X_CHD, X_S_DEGRID = PURIFY_X_SD, X_CH_GRID = PURIFY_X_CHG, X_S_GRID = PURIFY_X_SG;
+// TABLE mode: the table (R J/2 + 2 floats, 32 KB at R = 4096, J = 4) must stay resident in L1, which is what
+// the shared-memory carve-out leaves over.  Measured at config 5: grid 26.8 ms with a (4, 2) ring (table
+// evicted, every lookup an L2 access), 4.4 ms with (3, 2).  Smaller rings for the table kernels.
+constexpr int X_CH_DEGRID_T = 4, X_S_DEGRID_T = 2, X_CH_GRID_T = 3, X_S_GRID_T = 2;
 
 template <int J, int DEG> int launch_degrid_x_t(purify_op* op, void* y, cudaStream_t st) {
     typedef pk::XCfg<J> Cfg;
     if (op->n_items == 0) return PURIFY_OK;
-    const size_t smem = pk::XSmem<J, X_CH_DEGRID, X_S_DEGRID, false>::TOTAL;
+    size_t smem = pk::XSmem<J, X_CH_DEGRID, X_S_DEGRID, false>::TOTAL;
     const pk::XParams p = make_xparams(op, false);
     CK(cudaMemsetAsync(op->x_counter, 0, sizeof(unsigned), st));
     int g = 0, rc;
     if (op->mode == PURIFY_KERNEL_TABLE) {
-        auto kern = pk::degrid_x_kernel<J, DEG, 1, X_CH_DEGRID, X_S_DEGRID>;
+        smem = pk::XSmem<J, X_CH_DEGRID_T, X_S_DEGRID_T, false>::TOTAL;
+        auto kern = pk::degrid_x_kernel<J, DEG, 1, X_CH_DEGRID_T, X_S_DEGRID_T>;
         if ((rc = x_grid_size(kern, Cfg::THREADS, smem, op->n_items, Cfg::WARPS, &g))) return rc;
         kern<<<g, Cfg::THREADS, smem, st>>>(op->tmap_x, p, (float2*)y);
     } else {
@@ -256,12 +261,13 @@ template <int J, int DEG> int launch_degrid_x_t(purify_op* op, void* y, cudaStre
 template <int J, int DEG> int launch_grid_x_t(purify_op* op, const void* y, cudaStream_t st) {
     typedef pk::XCfg<J> Cfg;
     if (op->n_items == 0) return PURIFY_OK;
-    const size_t smem = pk::XSmem<J, X_CH_GRID, X_S_GRID, true>::TOTAL;
+    size_t smem = pk::XSmem<J, X_CH_GRID, X_S_GRID, true>::TOTAL;
     const pk::XParams p = make_xparams(op, false);
     CK(cudaMemsetAsync(op->x_counter, 0, sizeof(unsigned), st));
     int g = 0, rc;
     if (op->mode == PURIFY_KERNEL_TABLE) {
-        auto kern = pk::grid_x_kernel<J, DEG, 1, X_CH_GRID, X_S_GRID>;
+        smem = pk::XSmem<J, X_CH_GRID_T, X_S_GRID_T, true>::TOTAL;
+        auto kern = pk::grid_x_kernel<J, DEG, 1, X_CH_GRID_T, X_S_GRID_T>;
         if ((rc = x_grid_size(kern, Cfg::THREADS, smem, op->n_items, Cfg::WARPS, &g))) return rc;
         kern<<<g, Cfg::THREADS, smem, st>>>(p, (const float2*)y);
     } else {
