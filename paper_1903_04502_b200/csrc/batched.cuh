@@ -511,14 +511,21 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
                     rp += REC_FLOATS;
                     float2 g[J];
                     x_weights<J, DEG, MODE>(uvk, cellf, cx, cy, p, g);
-                    float2 acc = make_float2(0.f, 0.f);
+                    // J independent row chains (a dependent FFMA2 is J instructions away), two column chains
+                    float2 r[J];
 #pragma unroll
-                    for (int a = 0; a < J; ++a) {
-                        float2 row = mul2(dup2(g[0].x), B[a][0]);
+                    for (int a = 0; a < J; ++a) r[a] = mul2(dup2(g[0].x), B[a][0]);
 #pragma unroll
-                        for (int c = 1; c < J; ++c) row = fma2(dup2(g[c].x), B[a][c], row);
-                        acc = fma2(dup2(g[a].y), row, acc);
+                    for (int c = 1; c < J; ++c)
+#pragma unroll
+                        for (int a = 0; a < J; ++a) r[a] = fma2(dup2(g[c].x), B[a][c], r[a]);
+                    float2 acc0 = mul2(dup2(g[0].y), r[0]), acc1 = mul2(dup2(g[1].y), r[1]);
+#pragma unroll
+                    for (int a = 2; a < J; a += 2) {
+                        acc0 = fma2(dup2(g[a].y), r[a], acc0);
+                        acc1 = fma2(dup2(g[a + 1].y), r[a + 1], acc1);
                     }
+                    const float2 acc = add2(acc0, acc1);
                     *yout = mul2(dup2(wk), acc);                            // padding slots: w = 0 -> 0
                     yout += 32;
                 }
@@ -548,7 +555,7 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
 // one band meet there).
 template <int J, int DEG, int MODE, int CH, int S>
 __global__ void __launch_bounds__(XCfg<J>::THREADS)
-grid_x_kernel(const XParams p, const float2* __restrict__ y) {
+grid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, const float2* __restrict__ y) {
     typedef XCfg<J> Cfg;
     typedef RingCfg<CH, true> R;
     typedef XSmem<J, CH, S, true> SM;
@@ -584,6 +591,8 @@ grid_x_kernel(const XParams p, const float2* __restrict__ y) {
             }
         }
         int cnext = S;
+        if (lane == 0) bulk_wait_group_read0();         // the previous item's box reduction has read the box
+        __syncwarp();
         for (int i = lane; i < BOXW * BOXH; i += 32) tile[i] = make_float2(0.f, 0.f);
         __syncwarp();
         int left = T, rem = 0;
@@ -671,18 +680,30 @@ grid_x_kernel(const XParams p, const float2* __restrict__ y) {
                 __syncwarp();
             }
         }
-        // ---- add the box to the global grid (periodic wrap here)
+        // ---- add the box to the global grid: one TMA reduction (element-wise fp32 adds at L2) for a box in the
+        // interior, 8-byte reductions with periodic wrap for a box that crosses the grid edge.  Halos of
+        // neighbouring bands and the items of one band meet here.
         __syncwarp();
         const int bx0 = it.x0 - (J / 2 - 1) - XOFF, by0 = it.y0 - (J / 2 - 1);
-        for (int i = lane; i < BOXW * BOXH; i += 32) {
-            const float2 v = tile[i];
-            if (v.x != 0.f || v.y != 0.f) {
-                const int r = wrap_idx(by0 + i / BOXW, p.K, p.kmask), c = wrap_idx(bx0 + i % BOXW, p.K, p.kmask);
-                atomicAdd(p.grid + (long long)r * p.K + c, v);
+        const bool interior = bx0 >= 0 && by0 >= 0 && bx0 + BOXW <= p.K && by0 + BOXH <= p.K;
+        if (interior) {
+            if (lane == 0) {
+                fence_proxy_async();
+                tma_reduce_add_2d(&tmap, 2 * bx0, by0, tile);
+                bulk_commit_group();
+            }
+        } else {
+            for (int i = lane; i < BOXW * BOXH; i += 32) {
+                const float2 v = tile[i];
+                if (v.x != 0.f || v.y != 0.f) {
+                    const int r = wrap_idx(by0 + i / BOXW, p.K, p.kmask), c = wrap_idx(bx0 + i % BOXW, p.K, p.kmask);
+                    atomicAdd(p.grid + (long long)r * p.K + c, v);
+                }
             }
         }
         __syncwarp();
     }
+    if (lane == 0) bulk_wait_group_read0();             // shared memory must outlive the last reduction's reads
 }
 
 }  // namespace pk

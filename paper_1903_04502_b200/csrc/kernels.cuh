@@ -124,6 +124,15 @@ __device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* t
         ::"r"(smem_u32(smem_dst)), "l"(tmap), "r"(x), "r"(y), "r"(smem_u32(bar)) : "memory");
 }
 
+// TMA reduction: global[box at (x, y)] += smem box, element-wise fp32 adds performed at L2 (no return value)
+__device__ __forceinline__ void tma_reduce_add_2d(const CUtensorMap* tmap, int x, int y, const void* smem_src) {
+    asm volatile(
+        "cp.reduce.async.bulk.tensor.2d.global.shared::cta.add.tile.bulk_group [%0, {%1, %2}], [%3];"
+        ::"l"(tmap), "r"(x), "r"(y), "r"(smem_u32(smem_src)) : "memory");
+}
+__device__ __forceinline__ void bulk_commit_group() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_group_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+
 // ---------------------------------------------------------------------------------------------
 // a1: S + Z fused.  Writes the WHOLE K x K grid: b[p^ mod K] = sign s[py] s[px] x[py,px], 0 elsewhere,
 // with sign = (-1)^(p^x + p^y) so that the FFT output lands DC-centred (index c + K/2): the dense
@@ -276,6 +285,23 @@ __global__ void permute_kernel(const C* __restrict__ in, C* __restrict__ out, co
         if (to_native) { C z; z.x = 0; z.y = 0; out[k] = pi == 0xFFFFFFFFu ? z : in[pi]; }
         else if (pi != 0xFFFFFFFFu) out[pi] = in[k];
     }
+}
+
+// inverse of the native -> caller permutation (padding entries skipped): inv[perm[k]] = k
+__global__ void invert_perm_kernel(const unsigned* __restrict__ perm, long long M_native, unsigned* __restrict__ inv) {
+    for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < M_native; k += (long long)gridDim.x * blockDim.x) {
+        const unsigned pi = perm[k];
+        if (pi != 0xFFFFFFFFu) inv[pi] = (unsigned)k;
+    }
+}
+
+// native -> caller order as a GATHER (coalesced 8/16-byte stores, scattered loads): measurably cheaper than
+// the scatter form, whose partial-sector stores cost a read-modify-write each
+template <typename C>
+__global__ void gather_from_native_kernel(const C* __restrict__ in, C* __restrict__ out, const unsigned* __restrict__ inv,
+                                          long long M) {
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < M; i += (long long)gridDim.x * blockDim.x)
+        out[i] = in[inv[i]];
 }
 
 }  // namespace pk
