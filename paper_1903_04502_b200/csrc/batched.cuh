@@ -382,6 +382,15 @@ __device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gsrc, uint3
                  ::"r"(smem_u32(smem_dst)), "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
+__device__ __forceinline__ float2 lds_v2(uint32_t a) {
+    float2 v;
+    asm volatile("ld.volatile.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sts_v2(uint32_t a, float2 v) {
+    asm volatile("st.volatile.shared.v2.f32 [%0], {%1, %2};" ::"r"(a), "f"(v.x), "f"(v.y) : "memory");
+}
+
 template <int CH, bool WITH_Y> struct RingCfg {
     static constexpr int REC = CH * REC_BYTES, Y = WITH_Y ? CH * 256 : 0;
     static constexpr int STAGE = REC + Y;
@@ -660,13 +669,24 @@ grid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, const f
             // ---- flush the accumulators into the warp's box; idle lanes (no unit) stay out
             float2* dst = tile + ly * BOXW + lx + XOFF;
             if (!dup) {
+                // One read-modify-write per tap.  In step (a, c) the lanes touch distinct addresses (distinct
+                // cells); the footprints of different lanes overlap ACROSS steps, so step s+1 must see step s.
+                // The warp is converged here and the block below is straight-line code, so every lane issues
+                // each shared-memory instruction together and the LSU performs a warp's shared-memory
+                // instructions in issue order; the volatile asm keeps the compiler from reordering them.
+                // (A __syncwarp() per step is semantically the same and costs a BRA.DIV + NOP per tap.)
+                __syncwarp();
+                if (cnt > 0) {
+                    const uint32_t da = smem_u32(dst);
 #pragma unroll
-                for (int a = 0; a < J; ++a)
+                    for (int a = 0; a < J; ++a)
 #pragma unroll
-                    for (int c = 0; c < J; ++c) {
-                        if (cnt > 0) dst[a * BOXW + c] = add2(dst[a * BOXW + c], A[a][c]);
-                        __syncwarp();
-                    }
+                        for (int c = 0; c < J; ++c) {
+                            const uint32_t ad = da + (uint32_t)(a * BOXW + c) * 8u;
+                            sts_v2(ad, add2(lds_v2(ad), A[a][c]));
+                        }
+                }
+                __syncwarp();
             } else {
                 if (cnt > 0) {
 #pragma unroll
