@@ -423,7 +423,7 @@ __device__ __forceinline__ void ring_issue(unsigned char* ring, uint64_t* rbar, 
 // per batch every lane loads its cell's J x J patch into registers and then runs its unit's
 // visibilities out of registers.  HBM per slot: uv 8 + w 4 read, y 8 written (native order).
 template <int J, int DEG, int MODE, int CH, int S>
-__global__ void __launch_bounds__(XCfg<J>::THREADS)
+__global__ void __launch_bounds__(XCfg<J>::THREADS, J <= 6 ? 4 : 1)
 degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float2* __restrict__ y) {
     typedef XCfg<J> Cfg;
     typedef RingCfg<CH, false> R;
