@@ -259,3 +259,23 @@ def test_degrid_bit_reproducible_and_host_create():
     assert np.array_equal(host(op2.degrid(dev(x))), a)
     op.close()
     op2.close()
+
+
+def test_hot_cells_and_layer_straddling_batches():
+    """Batched complex64 layout: a handful of cells with hundreds of visibilities (several full units per cell,
+    layers of different widths, batches that straddle layer boundaries and hold one cell twice -> the flagged
+    flush path) on top of a sparse background."""
+    rng = synth.rng_for(4242, synth.STREAM_UV)
+    n, J = 64, 6
+    K = 2 * n
+    hot = rng.integers(-20, 20, size=(7, 2)).astype(np.float64)
+    counts = [700, 333, 129, 128, 65, 64, 63]
+    parts = [h + rng.uniform(0.0, 1.0, size=(c, 2)) for h, c in zip(hot, counts)]
+    parts.append(rng.uniform(-K / 2, K / 2, size=(3000, 2)))
+    uv = np.concatenate(parts)
+    uv = uv[rng.permutation(len(uv))]
+    w = rng.uniform(0.5, 1.5, size=len(uv))
+    x = synth.random_complex((n, n), seed=9)
+    info = run_all_checks(x, uv, w, J, "c64")
+    assert info["layout"] == 1
+    run_all_checks(x, uv, w, J, "c128")
