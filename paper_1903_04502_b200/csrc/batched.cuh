@@ -35,7 +35,16 @@ constexpr int XBW = 32, XBH = 16, XCELLS = XBW * XBH;   // band geometry
 constexpr int UNIT_CAP = 64;                            // visibilities per unit
 constexpr int ITEM_ITERS = 256;                         // iterations per item
 constexpr unsigned PERM_PAD = 0xFFFFFFFFu;
-constexpr int REC_FLOATS = 96, REC_BYTES = 384;         // per-iteration record: uv[32] | w[32]
+constexpr int REC_FLOATS = 96, REC_BYTES = 384;
+#ifndef PURIFY_XVD
+#define PURIFY_XVD 2
+#endif
+#ifndef PURIFY_XVG
+#define PURIFY_XVG 1
+#endif
+// visibilities per inner-loop trip (statement-interleaved dependency graphs): degridding gains from 2 (0.73 ->
+// 0.69 ms at config 4, 160 registers, 3 CTAs / SM); gridding loses (its flush phases want the 4th CTA)
+constexpr int XVD = PURIFY_XVD, XVG = PURIFY_XVG;         // per-iteration record: uv[32] | w[32]
 
 template <int J> struct XCfg {
     static constexpr int XOFF = (J / 2 - 1) & 1;        // makes the box's first column even (TMA: 16-byte aligned)
@@ -364,6 +373,95 @@ __device__ __forceinline__ void x_weights(float2 uv, float2 cellf, int cx, int c
     }
 }
 
+// Kernel weights of V visibilities of one cell, written statement-interleaved so that the V dependency
+// graphs advance together (ANALYTIC; TABLE evaluates visibility by visibility).
+template <int J, int DEG, int MODE, int V>
+__device__ __forceinline__ void x_weights_v(const float2 (&uv)[V], float2 cellf, int cx, int cy, const XParams& p,
+                                            float2 (&g)[V][J]) {
+    if (MODE == 0) {
+        constexpr int NE = DEG / 2 + 1, NO = (DEG + 1) / 2;
+        float2 t[V], t2[V], nt[V];
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+            t[v] = add2(add2(uv[v], make_float2(-cellf.x, -cellf.y)), make_float2(-0.5f, -0.5f));
+            t2[v] = mul2(t[v], t[v]);
+            nt[v] = make_float2(-t[v].x, -t[v].y);
+        }
+#pragma unroll
+        for (int j = 0; j < J / 2; ++j) {
+            float2 E[V], O[V];
+#pragma unroll
+            for (int v = 0; v < V; ++v) { E[v] = dup2(p.coef.e[j][NE - 1]); O[v] = dup2(p.coef.o[j][NO - 1]); }
+#pragma unroll
+            for (int m = NE - 2; m >= 0; --m)
+#pragma unroll
+                for (int v = 0; v < V; ++v) E[v] = fma2(E[v], t2[v], dup2(p.coef.e[j][m]));
+#pragma unroll
+            for (int m = NO - 2; m >= 0; --m)
+#pragma unroll
+                for (int v = 0; v < V; ++v) O[v] = fma2(O[v], t2[v], dup2(p.coef.o[j][m]));
+#pragma unroll
+            for (int v = 0; v < V; ++v) { g[v][j] = fma2(t[v], O[v], E[v]); g[v][J - 1 - j] = fma2(nt[v], O[v], E[v]); }
+        }
+    } else {
+#pragma unroll
+        for (int v = 0; v < V; ++v) x_weights<J, DEG, MODE>(uv[v], cellf, cx, cy, p, g[v]);
+    }
+}
+
+// a3 arithmetic for V visibilities of one cell: J independent row chains per visibility (a dependent FFMA2 is
+// V J instructions away), two column chains.
+template <int J, int DEG, int MODE, int V>
+__device__ __forceinline__ void x_degrid_vis(const float2 (&uv)[V], const float (&w)[V], float2 cellf, int cx, int cy,
+                                             const XParams& p, const float2 (&B)[J][J], float2 (&out)[V]) {
+    float2 g[V][J];
+    x_weights_v<J, DEG, MODE, V>(uv, cellf, cx, cy, p, g);
+    float2 r[V][J];
+#pragma unroll
+    for (int a = 0; a < J; ++a)
+#pragma unroll
+        for (int v = 0; v < V; ++v) r[v][a] = mul2(dup2(g[v][0].x), B[a][0]);
+#pragma unroll
+    for (int c = 1; c < J; ++c)
+#pragma unroll
+        for (int a = 0; a < J; ++a)
+#pragma unroll
+            for (int v = 0; v < V; ++v) r[v][a] = fma2(dup2(g[v][c].x), B[a][c], r[v][a]);
+    float2 acc0[V], acc1[V];
+#pragma unroll
+    for (int v = 0; v < V; ++v) { acc0[v] = mul2(dup2(g[v][0].y), r[v][0]); acc1[v] = mul2(dup2(g[v][1].y), r[v][1]); }
+#pragma unroll
+    for (int a = 2; a < J; a += 2)
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+            acc0[v] = fma2(dup2(g[v][a].y), r[v][a], acc0[v]);
+            acc1[v] = fma2(dup2(g[v][a + 1].y), r[v][a + 1], acc1[v]);
+        }
+#pragma unroll
+    for (int v = 0; v < V; ++v) out[v] = mul2(dup2(w[v]), add2(acc0[v], acc1[v]));      // padding slots: w = 0 -> 0
+}
+
+// a4 arithmetic for V visibilities of one cell: A[a][c] += g_x[c] (g_y[a] w y), visibility by visibility per tap
+template <int J, int DEG, int MODE, int V>
+__device__ __forceinline__ void x_grid_vis(const float2 (&uv)[V], const float (&w)[V], const float2 (&yv)[V], float2 cellf,
+                                           int cx, int cy, const XParams& p, float2 (&A)[J][J]) {
+    float2 g[V][J];
+    x_weights_v<J, DEG, MODE, V>(uv, cellf, cx, cy, p, g);
+    float2 z[V];
+#pragma unroll
+    for (int v = 0; v < V; ++v) z[v] = mul2(dup2(w[v]), yv[v]);
+#pragma unroll
+    for (int a = 0; a < J; ++a) {
+        float2 q[V];
+#pragma unroll
+        for (int v = 0; v < V; ++v) q[v] = mul2(dup2(g[v][a].y), z[v]);
+#pragma unroll
+        for (int v = 0; v < V; ++v)
+#pragma unroll
+            for (int c = 0; c < J; ++c) A[a][c] = fma2(dup2(g[v][c].x), q[v], A[a][c]);
+    }
+}
+
 __device__ __forceinline__ unsigned x_next_item(unsigned* counter, int lane) {
     unsigned it = 0;
     if (lane == 0) it = atomicAdd(counter, 1u);
@@ -423,7 +521,7 @@ __device__ __forceinline__ void ring_issue(unsigned char* ring, uint64_t* rbar, 
 // per batch every lane loads its cell's J x J patch into registers and then runs its unit's
 // visibilities out of registers.  HBM per slot: uv 8 + w 4 read, y 8 written (native order).
 template <int J, int DEG, int MODE, int CH, int S>
-__global__ void __launch_bounds__(XCfg<J>::THREADS, J <= 6 ? 4 : 1)
+__global__ void __launch_bounds__(XCfg<J>::THREADS, J <= 6 ? (XVD == 1 ? 4 : (XVD == 2 ? 3 : 2)) : 1)
 degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float2* __restrict__ y) {
     typedef XCfg<J> Cfg;
     typedef RingCfg<CH, false> R;
@@ -513,29 +611,29 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
                     rp = reinterpret_cast<const float*>(ring + stage * R::STAGE) + lane;
                 }
                 const int seg = min(rem, n_iter - i);
+                int k = 0;
 #pragma unroll 1
-                for (int k = 0; k < seg; ++k) {
-                    const float2 uvk = *reinterpret_cast<const float2*>(rp + lane);
-                    const float wk = rp[64];
-                    rp += REC_FLOATS;
-                    float2 g[J];
-                    x_weights<J, DEG, MODE>(uvk, cellf, cx, cy, p, g);
-                    // J independent row chains (a dependent FFMA2 is J instructions away), two column chains
-                    float2 r[J];
+                for (; k + XVD <= seg; k += XVD) {            // XVD visibilities per trip: XVD interleaved dependency graphs
+                    float2 uvk[XVD], o[XVD];
+                    float wk[XVD];
 #pragma unroll
-                    for (int a = 0; a < J; ++a) r[a] = mul2(dup2(g[0].x), B[a][0]);
-#pragma unroll
-                    for (int c = 1; c < J; ++c)
-#pragma unroll
-                        for (int a = 0; a < J; ++a) r[a] = fma2(dup2(g[c].x), B[a][c], r[a]);
-                    float2 acc0 = mul2(dup2(g[0].y), r[0]), acc1 = mul2(dup2(g[1].y), r[1]);
-#pragma unroll
-                    for (int a = 2; a < J; a += 2) {
-                        acc0 = fma2(dup2(g[a].y), r[a], acc0);
-                        acc1 = fma2(dup2(g[a + 1].y), r[a + 1], acc1);
+                    for (int v = 0; v < XVD; ++v) {
+                        uvk[v] = *reinterpret_cast<const float2*>(rp + v * REC_FLOATS + lane);
+                        wk[v] = rp[v * REC_FLOATS + 64];
                     }
-                    const float2 acc = add2(acc0, acc1);
-                    *yout = mul2(dup2(wk), acc);                            // padding slots: w = 0 -> 0
+                    rp += XVD * REC_FLOATS;
+                    x_degrid_vis<J, DEG, MODE, XVD>(uvk, wk, cellf, cx, cy, p, B, o);
+#pragma unroll
+                    for (int v = 0; v < XVD; ++v) yout[v * 32] = o[v];
+                    yout += XVD * 32;
+                }
+                for (; XVD > 1 && k < seg; ++k) {            // tail of the segment, one visibility at a time
+                    const float2 uv1[1] = {*reinterpret_cast<const float2*>(rp + lane)};
+                    const float w1[1] = {rp[64]};
+                    float2 o1[1];
+                    rp += REC_FLOATS;
+                    x_degrid_vis<J, DEG, MODE, 1>(uv1, w1, cellf, cx, cy, p, B, o1);
+                    *yout = o1[0];
                     yout += 32;
                 }
                 i += seg;
@@ -563,7 +661,7 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
 // 8-byte reduction per non-zero cell (RED.ADD.F32x2; halos of neighbouring bands and the items of
 // one band meet there).
 template <int J, int DEG, int MODE, int CH, int S>
-__global__ void __launch_bounds__(XCfg<J>::THREADS)
+__global__ void __launch_bounds__(XCfg<J>::THREADS, J <= 6 ? (XVG == 1 ? 4 : 3) : 1)
 grid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, const float2* __restrict__ y) {
     typedef XCfg<J> Cfg;
     typedef RingCfg<CH, true> R;
@@ -637,23 +735,30 @@ grid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, const f
                 }
                 const int seg = min(rem, n_iter - i);
                 int live = cnt - i;                                         // slots of this segment that hold a visibility
+                int k = 0;
 #pragma unroll 1
-                for (int k = 0; k < seg; ++k, --live) {
-                    const float2 uvk = *reinterpret_cast<const float2*>(rp + lane);
-                    const float wk = rp[64];
-                    float2 yk = *yp;
+                for (; k + XVG <= seg; k += XVG, live -= XVG) {
+                    float2 uvk[XVG], yk[XVG];
+                    float wk[XVG];
+#pragma unroll
+                    for (int v = 0; v < XVG; ++v) {
+                        uvk[v] = *reinterpret_cast<const float2*>(rp + v * REC_FLOATS + lane);
+                        wk[v] = rp[v * REC_FLOATS + 64];
+                        yk[v] = yp[v * 32];
+                        if (live <= v) yk[v] = make_float2(0.f, 0.f);       // padding slot: whatever y holds there is ignored
+                    }
+                    rp += XVG * REC_FLOATS;
+                    yp += XVG * 32;
+                    x_grid_vis<J, DEG, MODE, XVG>(uvk, wk, yk, cellf, cx, cy, p, A);
+                }
+                for (; XVG > 1 && k < seg; ++k, --live) {
+                    const float2 uv1[1] = {*reinterpret_cast<const float2*>(rp + lane)};
+                    const float w1[1] = {rp[64]};
+                    float2 y1[1] = {*yp};
+                    if (live <= 0) y1[0] = make_float2(0.f, 0.f);
                     rp += REC_FLOATS;
                     yp += 32;
-                    if (live <= 0) yk = make_float2(0.f, 0.f);              // padding slot: whatever y holds there is ignored
-                    float2 g[J];
-                    x_weights<J, DEG, MODE>(uvk, cellf, cx, cy, p, g);
-                    const float2 z = mul2(dup2(wk), yk);
-#pragma unroll
-                    for (int a = 0; a < J; ++a) {
-                        const float2 q = mul2(dup2(g[a].y), z);
-#pragma unroll
-                        for (int c = 0; c < J; ++c) A[a][c] = fma2(dup2(g[c].x), q, A[a][c]);
-                    }
+                    x_grid_vis<J, DEG, MODE, 1>(uv1, w1, y1, cellf, cx, cy, p, A);
                 }
                 i += seg;
                 rem -= seg;
