@@ -227,7 +227,7 @@ template <typename Kern> int x_grid_size(Kern kern, int threads, size_t smem, in
 // ring geometry of the complex64 kernels: CH iterations per chunk, S stages (batched.cuh "ring")
 // ring geometry (chunk iterations, stages) of the two complex64 kernels; -D overrides are for tuning builds
 #ifndef PURIFY_X_CHD
-#define PURIFY_X_CHD 8
+#define PURIFY_X_CHD 16
 #define PURIFY_X_SD 2
 #define PURIFY_X_CHG 6
 #define PURIFY_X_SG 2
