@@ -123,7 +123,9 @@ int purify_grid(purify_op *op, const void *y_dev, void *x_dev, void *cuda_stream
 int purify_normal(purify_op *op, const void *x_in_dev, void *x_out_dev, void *cuda_stream);
 
 /* Same operators with y in NATIVE order (moves only the minimum bytes; an ADMM loop can keep all
- * its M-sized vectors in this order after one purify_permute_to_native of the data). */
+ * its M-sized vectors in this order after one purify_permute_to_native of the data).  Native vectors have
+ * M_native entries (purify_op_info); for PURIFY_C64 the y_native pointer given to purify_grid_native must be
+ * 16-byte aligned (INVALID_ARG otherwise: the kernel streams it with bulk copies). */
 int purify_degrid_native(purify_op *op, const void *x_dev, void *y_native_dev, void *cuda_stream);
 int purify_grid_native(purify_op *op, const void *y_native_dev, void *x_dev, void *cuda_stream);
 int purify_permute_to_native(purify_op *op, const void *y_caller_dev, void *y_native_dev, void *cuda_stream);

@@ -10,6 +10,7 @@
 #include <cufft.h>
 
 #include <cstdarg>
+#include <cstdint>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -917,6 +918,8 @@ int purify_grid(purify_op* op, const void* y_dev, void* x_dev, void* cuda_stream
 
 int purify_grid_native(purify_op* op, const void* y_native_dev, void* x_dev, void* cuda_stream) {
     NEED_OP(op); NEED_PTR(x_dev, "x"); if (op->M > 0) NEED_PTR(y_native_dev, "y");
+    if (op->batched && ((uintptr_t)y_native_dev & 15u))       // the kernel streams y with 16-byte-aligned bulk copies
+        return fail(PURIFY_ERR_INVALID_ARG, "y_native must be 16-byte aligned for the complex64 layout");
     begin_call(op);
     return grid_impl(op, y_native_dev, x_dev, false, (cudaStream_t)cuda_stream);
 }

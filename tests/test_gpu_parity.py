@@ -245,6 +245,15 @@ def test_errors():
     with pytest.raises(ValueError):
         op.degrid(torch.zeros((16, 16), dtype=torch.complex128, device="cuda"))
     op.close()
+    # complex64 layout: native-order y must be 16-byte aligned (it is streamed by bulk copies)
+    uv32 = torch.rand((100, 2), dtype=torch.float32, device="cuda") * 8 - 4
+    op = PurifyOp(32, 4, uv32, None, dtype=C64)
+    buf = torch.zeros(op.M_native + 1, dtype=torch.complex64, device="cuda")
+    with pytest.raises(PurifyError) as ei:
+        op.grid(buf[1:], native=True)
+    assert ei.value.status == -1
+    op.grid(buf[:-1], native=True)
+    op.close()
 
 
 def test_degrid_bit_reproducible_and_host_create():
