@@ -24,7 +24,7 @@
 //          batch.  Slots past a unit's count are padding: perm = 0xFFFFFFFF, w = 0, uv = the unit's
 //          first visibility, y_native = 0.  The per-slot inputs are stored as one record per
 //          ITERATION: 32 x (u, v) then 32 x w = 384 bytes, so a chunk of iterations is ONE bulk copy.
-//   item   a run of batches of one band with about ITEM_ITERS iterations: the unit of dynamic
+//   item   a run of batches of one band with about ITEM_ITERS (64) iterations: the unit of dynamic
 //          scheduling (persistent warps pull items from an atomic counter); its slots are contiguous.
 #pragma once
 #include "kernels.cuh"
@@ -33,7 +33,10 @@ namespace pk {
 
 constexpr int XBW = 32, XBH = 16, XCELLS = XBW * XBH;   // band geometry
 constexpr int UNIT_CAP = 64;                            // visibilities per unit
-constexpr int ITEM_ITERS = 256;                         // iterations per item
+#ifndef PURIFY_ITEM_ITERS
+#define PURIFY_ITEM_ITERS 64
+#endif
+constexpr int ITEM_ITERS = PURIFY_ITEM_ITERS;                         // iterations per item
 constexpr unsigned PERM_PAD = 0xFFFFFFFFu;
 constexpr int REC_FLOATS = 96, REC_BYTES = 384;
 #ifndef PURIFY_XVD
@@ -137,7 +140,7 @@ band_build_kernel(const unsigned* __restrict__ keys, const unsigned* __restrict_
                   XItem* __restrict__ items) {
     __shared__ unsigned s_rem[XCELLS], s_remsorted[XCELLS], s_scan[XCELLS], s_ni[XCELLS];
     __shared__ unsigned s_w[XCELLS / 32];
-    __shared__ unsigned s_F, s_Rn, s_maxfull, s_carry, s_lastni;
+    __shared__ unsigned s_F, s_Rn, s_maxfull, s_carry, s_lastni, s_icarry;
 
     const int band = blockIdx.x;
     const unsigned bs = band_start[band], be = band_start[band + 1];
@@ -146,7 +149,7 @@ band_build_kernel(const unsigned* __restrict__ keys, const unsigned* __restrict_
         if (PASS == 1 && t == 0) { totals[band].nb = 0; totals[band].iters = 0; totals[band].items = 0; }
         return;
     }
-    if (t == 0) { s_F = 0; s_Rn = 0; s_maxfull = 0; s_carry = 0; s_lastni = 0; }
+    if (t == 0) { s_F = 0; s_Rn = 0; s_maxfull = 0; s_carry = 0; s_lastni = 0; s_icarry = 0; }
     // --- this cell's visibilities: [start, start + cnt) of the sorted order
     unsigned start, cnt;
     {
@@ -180,29 +183,33 @@ band_build_kernel(const unsigned* __restrict__ keys, const unsigned* __restrict_
                    item0 = PASS == 2 ? item_off[band] : 0;
     const int x0 = (band % nbx) * XBW, y0 = (band / nbx) * XBH;
 
-    // --- batches: n_iter, prefix of iterations, item boundaries (chunks of 512 batches)
+    // --- batches: n_iter, prefix of iterations, item boundaries (chunks of 512 batches).  A batch opens a new
+    // item when the iterations before it cross a multiple of ITEM_ITERS; items are numbered by a scan of these flags.
+    auto block_scan = [&](unsigned v) -> unsigned {          // inclusive scan over the CTA's 512 threads
+        s_scan[t] = v;
+        __syncthreads();
+        for (int off = 1; off < XCELLS; off <<= 1) {
+            const unsigned u = t >= off ? s_scan[t - off] : 0;
+            __syncthreads();
+            s_scan[t] += u;
+            __syncthreads();
+        }
+        const unsigned r = s_scan[t];
+        __syncthreads();
+        return r;
+    };
     unsigned total_iters = 0;
     for (unsigned base = 0; base < NB; base += XCELLS) {
         const unsigned b = base + t;
         const unsigned ni = b < NB ? batch_iters(b) : 0u;
         s_ni[t] = ni;
-        s_scan[t] = ni;
-        __syncthreads();
-        for (int off = 1; off < XCELLS; off <<= 1) {
-            const unsigned v = t >= off ? s_scan[t - off] : 0;
-            __syncthreads();
-            s_scan[t] += v;
-            __syncthreads();
-        }
-        const unsigned carry = s_carry;
-        const unsigned incl = s_scan[t] + carry, excl = incl - ni;
+        const unsigned incl = block_scan(ni) + s_carry, excl = incl - ni;
+        const unsigned ni_prev = t > 0 ? s_ni[t - 1] : s_lastni;
+        const bool first = b < NB && (b == 0 || excl / ITEM_ITERS != (excl - ni_prev) / ITEM_ITERS);
+        const unsigned fincl = block_scan(first ? 1u : 0u) + s_icarry;
         if (PASS == 2 && b < NB) {
+            const unsigned item = fincl - 1;
             bhdr[nb0 + b] = make_uint2(it0 + excl, ni);                 // flags are OR-ed in below
-            // item of a batch = floor(iterations before it / ITEM_ITERS); a batch opens an item when
-            // its predecessor belongs to another one
-            const unsigned item = excl / ITEM_ITERS;
-            const unsigned ni_prev = t > 0 ? s_ni[t - 1] : s_lastni;
-            const bool first = b == 0 || item != (excl - ni_prev) / ITEM_ITERS;
             if (first) {
                 items[item0 + item].x0 = x0;
                 items[item0 + item].y0 = y0;
@@ -213,7 +220,7 @@ band_build_kernel(const unsigned* __restrict__ keys, const unsigned* __restrict_
             if (b == NB - 1) items[item0 + item].end = (int)(nb0 + NB);
         }
         __syncthreads();
-        if (t == XCELLS - 1) { s_carry = incl; s_lastni = ni; }
+        if (t == XCELLS - 1) { s_carry = incl; s_lastni = ni; s_icarry = fincl; }
         __syncthreads();
         total_iters = s_carry;
     }
@@ -221,8 +228,7 @@ band_build_kernel(const unsigned* __restrict__ keys, const unsigned* __restrict_
         if (t == 0) {
             totals[band].nb = NB;
             totals[band].iters = total_iters;
-            // items = distinct values of floor(excl(b) / ITEM_ITERS); excl of the last batch = total - n_iter(last)
-            totals[band].items = (total_iters - batch_iters(NB - 1)) / ITEM_ITERS + 1;
+            totals[band].items = s_icarry;
         }
         return;
     } else {
