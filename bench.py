@@ -173,6 +173,26 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def alu_roofline(cfg, M, stage_ms):
+    """fp32 FMA work of W G / G^dagger W^dagger per visibility (ANALYTIC mode): the J x J complex-times-real MACs
+    (2 J^2 + 2 J FMA for degridding, 2 J^2 + 2 J + 2 for gridding) plus the paired even/odd Horner chains of the
+    kernel weights, 2 axes x J/2 pairs x (deg + 1) FMA + 6; TABLE mode: the MACs only.  Peak: nominal plain-ALU fp32."""
+    if cfg.dtype != "c64":
+        return None
+    J = cfg.J
+    deg = 8 if J == 4 else 7
+    wts = 0 if cfg.kernel_mode == "table" else 2 * (J // 2) * (deg + 1) + 6
+    fma = {"degrid": 2 * J * J + 2 * J + 2 + wts, "grid": 2 * J * J + 2 * J + 2 + wts}
+    peak = 148 * 128 * 2 * 1.965e9 / 1e12
+    out = {"bound": "alu", "unit": "TFLOP/s", "peak": peak,
+           "peak_source": "nominal: 148 SMs x 128 fp32 lanes x 2 flop x 1.965 GHz (DESIGN.md 5)"}
+    for k, f in fma.items():
+        if stage_ms.get(k):
+            ach = 2.0 * f * M / (stage_ms[k] * 1e-3) / 1e12
+            out[k] = {"fma_per_visibility": f, "achieved": ach, "frac": ach / peak}
+    return out
+
+
 def workload(cfg, M, gpus):
     return {"workload": f"BASELINE.json configs[{cfg.index - 1}] ({cfg.name}): {cfg.n}x{cfg.n} image, "
                         f"{cfg.K}x{cfg.K} grid, Kaiser-Bessel J={cfg.J}, M={M} visibilities per GPU, "
@@ -243,12 +263,16 @@ def run_ours(args):
     barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
+    marks = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     e0.record()
-    for _ in range(args.steps):
+    marks[0].record()
+    for i in range(args.steps):
         step()
+        marks[i + 1].record()          # per-step marks (no synchronisation): mean / std / min as the paper reports
     e1.record()
     barrier()
     ms_total = e0.elapsed_time(e1)
+    per_step = [marks[i].elapsed_time(marks[i + 1]) for i in range(args.steps)]
     launches = op.last_launch_count() * args.steps
     ms_total = pdist.max_over_ranks(ms_total, device="cuda")
     ms_step = ms_total / args.steps
@@ -313,6 +337,8 @@ def run_ours(args):
         line = {
             "metric": METRIC, "value": world * M / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step,
+            "ms_per_step_stats": {"mean": statistics.mean(per_step), "std": statistics.pstdev(per_step), "min": min(per_step),
+                                  "max": max(per_step), "note": "rank 0, per-step CUDA events inside the timed region"},
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32" if cfg.dtype == "c64" else "f64", "data": "synthetic",
             "config": workload(cfg, M, world),
@@ -328,6 +354,10 @@ def run_ours(args):
                          "other_kernel": {k: {"ms": stage_ms[k], "achieved": alg_bytes / (stage_ms[k] * 1e-3) / 1e9,
                                               "frac": alg_bytes / (stage_ms[k] * 1e-3) / 1e9 / peak}
                                           for k in ("degrid", "grid") if k != dom}},
+            # the same kernels against the plain-ALU fp32 ceiling (they are FMA-bound, not HBM-bound):
+            # algorithmic flops = M x (4 J^2 + 4 J complex-times-real MAC flops + weight evaluation), peak = 148 SMs x
+            # 128 fp32 lanes x 2 flop x 1.965 GHz
+            "roofline_alu": alu_roofline(cfg, M, stage_ms),
             "stage_ms": stage_ms,
             "operators": {"phi_ms": ms_phi, "phi_vis_per_s": M / (ms_phi * 1e-3),
                           "phi_dagger_ms": ms_phit, "phi_dagger_vis_per_s": M / (ms_phit * 1e-3),
