@@ -307,6 +307,13 @@ def run_ours(args):
     ms_phit_caller = timed(lambda: op.grid(y_call, out_dev, native=False), reps)
     del y_call
 
+    # ---- f2: power method on Phi^dagger Phi, 10 iterations from the all-ones vector
+    t0 = time.perf_counter()
+    lam, its = op.norm(None, max_iter=10, rel_tol=0.0)
+    torch.cuda.synchronize()
+    norm_info = {"lambda_after_10_iterations": lam, "ms_per_iteration": (time.perf_counter() - t0) * 1e3 / max(its, 1),
+                 "note": "purify_op_norm: Phi^dagger Phi + fp64 norm + scaling per iteration, host-synchronised every iteration"}
+
     # ---- end to end through the C ABI with HOST buffers (H2D of x, D2H of the result inside)
     op.normal_host(x_pin, out_pin)
     barrier()
@@ -362,6 +369,7 @@ def run_ours(args):
             "operators": {"phi_ms": ms_phi, "phi_vis_per_s": M / (ms_phi * 1e-3),
                           "phi_dagger_ms": ms_phit, "phi_dagger_vis_per_s": M / (ms_phit * 1e-3),
                           "phi_caller_order_ms": ms_phi_caller, "phi_dagger_caller_order_ms": ms_phit_caller},
+            "operator_norm": norm_info,
             "clocks": clocks,
             "setup": {"generate_s": t_gen, "create_s": t_create, "n_items": info["n_items"],
                       "n_tiles_nonempty": info["n_tiles_nonempty"], "max_tile_count": info["max_tile_count"],

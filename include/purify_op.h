@@ -136,6 +136,15 @@ int purify_degrid_host(purify_op *op, const void *x_host, void *y_host, void *cu
 int purify_grid_host(purify_op *op, const void *y_host, void *x_host, void *cuda_stream);
 int purify_normal_host(purify_op *op, const void *x_in_host, void *x_out_host, void *cuda_stream);
 
+/* f2: largest eigenvalue of Phi^dagger Phi = ||Phi||^2 by the power method ("We can normalize the
+ * operator with the operator norm, by using the power method to estimate the largest eigenvalue").
+ * x_1 = x0 / ||x0||; z_k = Phi^dagger Phi x_k; lambda_k = ||z_k||_2; x_{k+1} = z_k / lambda_k; stops after max_iter
+ * iterations or when |lambda_k - lambda_{k-1}| <= rel_tol lambda_k (k >= 2; rel_tol = 0: run max_iter iterations).
+ * x0_dev: n*n complex start vector on the device, or NULL for all ones.  Norms are accumulated in fp64.
+ * lambda_out, iters_out: HOST pointers (iters_out may be NULL).  Synchronises the stream every iteration. */
+int purify_op_norm(purify_op *op, const void *x0_dev, int max_iter, double rel_tol, double *lambda_out, int *iters_out,
+                   void *cuda_stream);
+
 /* Stage access for tests (device pointers): the K x K Fourier grid workspace in the library's
  * internal layout is NOT exposed; these run single stages into caller buffers in the mathematical
  * layout B[ky*K + kx], ky, kx in [0, K) (DC at index 0), so they can be compared with the oracle. */

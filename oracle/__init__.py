@@ -205,3 +205,23 @@ def grid(y, uv, w, n, J, mode="analytic", R=4096, idx_prec=64) -> np.ndarray:
     lib().oracle_grid(int(n), int(J), uv.shape[0], y.view(np.float64).ctypes.data_as(_dp), _p(uv), _p(w),
                       _mode(mode), int(R), int(idx_prec), x.view(np.float64).ctypes.data_as(_dp))
     return x
+
+
+def power_method(x0, uv, w, n, J, max_iter=100, rel_tol=1e-6, mode="analytic", R=4096, idx_prec=64):
+    """f2: largest eigenvalue of Phi^dagger Phi by the power method, step by step:
+    x_1 = x0/||x0||; z_k = Phi^dagger Phi x_k; lambda_k = ||z_k||_2; x_{k+1} = z_k/lambda_k; stop after max_iter
+    iterations or when |lambda_k - lambda_{k-1}| <= rel_tol lambda_k (k >= 2).  x0 None = all ones.
+    Returns (lambda, iterations).  Pinned against numpy's dense eigen-solver on a tiny operator (tests)."""
+    x = np.ones((n, n), dtype=np.complex128) if x0 is None else _c128(x0).copy()
+    nrm = float(np.linalg.norm(x))
+    assert nrm > 0.0
+    lam = prev = 0.0
+    it = 0
+    for it in range(1, int(max_iter) + 1):
+        x = x / nrm
+        z = grid(degrid(x, uv, w, J, mode, R, idx_prec), uv, w, n, J, mode, R, idx_prec)
+        prev, lam = lam, float(np.linalg.norm(z))
+        x, nrm = z, lam
+        if not lam > 0.0 or (it > 1 and abs(lam - prev) <= rel_tol * lam):
+            break
+    return lam, it

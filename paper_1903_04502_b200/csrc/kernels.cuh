@@ -304,4 +304,39 @@ __global__ void gather_from_native_kernel(const C* __restrict__ in, C* __restric
         out[i] = in[inv[i]];
 }
 
+// ---------------------------------------------------------------------------------------------
+// f2: pieces of the power method on Phi^dagger Phi.
+// sum of |x_i|^2 over a complex vector, accumulated in fp64 into *out (zeroed by the caller)
+template <typename R>
+__global__ void __launch_bounds__(256) norm2_kernel(const typename Cplx<R>::type* __restrict__ x, long long count,
+                                                    double* __restrict__ out) {
+    double acc = 0.0;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < count; i += (long long)gridDim.x * blockDim.x) {
+        const typename Cplx<R>::type v = x[i];
+        acc += (double)v.x * (double)v.x + (double)v.y * (double)v.y;
+    }
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);
+    __shared__ double part[8];
+    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < 8; ++w) t += part[w];
+        atomicAdd(out, t);
+    }
+}
+
+// y = x / sqrt(*norm2) (y may alias x); a zero vector is left unchanged
+template <typename R>
+__global__ void __launch_bounds__(256) normalise_kernel(const typename Cplx<R>::type* __restrict__ x,
+                                                        typename Cplx<R>::type* __restrict__ y, long long count,
+                                                        const double* __restrict__ norm2) {
+    const double n2 = *norm2;
+    const double f = n2 > 0.0 ? 1.0 / sqrt(n2) : 1.0;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < count; i += (long long)gridDim.x * blockDim.x) {
+        const typename Cplx<R>::type v = x[i];
+        y[i] = mk2<R>((R)((double)v.x * f), (R)((double)v.y * f));
+    }
+}
+
 }  // namespace pk

@@ -9,6 +9,7 @@
 #include <cuda_runtime.h>
 #include <cufft.h>
 
+#include <cmath>
 #include <cstdarg>
 #include <cstdint>
 #include <cstdio>
@@ -87,6 +88,7 @@ struct purify_op {
     void* y_ws = nullptr;     // M complex (purify_normal / host paths), lazily allocated
     void* x_ws = nullptr;     // n*n complex staging for host paths
     void* y_ws2 = nullptr;    // caller-order staging for host paths
+    double* scal_ws = nullptr; // one fp64 scalar (norms)
     cufftHandle plan = 0;
     bool plan_ok = false;
     CUtensorMap tmap;
@@ -842,7 +844,7 @@ int purify_op_create_host(purify_op** out, int n, int oversample, int J, long lo
 
 int purify_op_destroy(purify_op* op) {
     if (!op) return PURIFY_OK;
-    cudaFree(op->grid); cudaFree(op->uv_s); cudaFree(op->w_s); cudaFree(op->perm); cudaFree(op->inv_perm); cudaFree(op->items);
+    cudaFree(op->grid); cudaFree(op->uv_s); cudaFree(op->w_s); cudaFree(op->perm); cudaFree(op->inv_perm); cudaFree(op->scal_ws); cudaFree(op->items);
     cudaFree(op->corr); cudaFree(op->table); cudaFree(op->y_ws); cudaFree(op->x_ws); cudaFree(op->y_ws2);
     cudaFree(op->x_bhdr); cudaFree(op->x_blane); cudaFree(op->x_items); cudaFree(op->x_counter);
     if (op->plan_ok) cufftDestroy(op->plan);
@@ -987,6 +989,65 @@ int purify_normal_host(purify_op* op, const void* x_in_host, void* x_out_host, v
     RUN(grid_impl(op, op->y_ws, op->x_ws, false, st));
     CK(cudaMemcpyAsync(x_out_host, op->x_ws, xb, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
+    return PURIFY_OK;
+}
+
+// ---- f2: operator norm by the power method
+int purify_op_norm(purify_op* op, const void* x0_dev, int max_iter, double rel_tol, double* lambda_out, int* iters_out,
+                   void* cuda_stream) {
+    NEED_OP(op); NEED_PTR(lambda_out, "lambda_out");
+    if (max_iter < 1) return fail(PURIFY_ERR_INVALID_ARG, "max_iter must be >= 1 (got %d)", max_iter);
+    if (!(rel_tol >= 0.0)) return fail(PURIFY_ERR_INVALID_ARG, "rel_tol must be >= 0");
+    begin_call(op);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const long long N = (long long)op->n * op->n;
+    const size_t xb = csize(op) * (size_t)N;
+    RUN(ensure_ws(op, &op->x_ws, xb));
+    RUN(ensure_ws(op, &op->y_ws, csize(op) * (size_t)op->M_native));
+    RUN(ensure_ws(op, (void**)&op->scal_ws, sizeof(double)));
+    const bool f32 = op->dtype == PURIFY_C64;
+    auto norm2 = [&](const void* v, double* host) -> int {
+        CK(cudaMemsetAsync(op->scal_ws, 0, sizeof(double), st));
+        if (f32) pk::norm2_kernel<float><<<grid_for(N, 256, 148 * 8), 256, 0, st>>>((const float2*)v, N, op->scal_ws);
+        else pk::norm2_kernel<double><<<grid_for(N, 256, 148 * 8), 256, 0, st>>>((const double2*)v, N, op->scal_ws);
+        op->launches++;
+        CK(cudaGetLastError());
+        if (host) { CK(cudaMemcpyAsync(host, op->scal_ws, sizeof(double), cudaMemcpyDeviceToHost, st)); CK(cudaStreamSynchronize(st)); }
+        return PURIFY_OK;
+    };
+    auto normalise = [&]() -> int {                    // x_ws <- x_ws / sqrt(scal_ws)
+        if (f32) pk::normalise_kernel<float><<<grid_for(N, 256, 148 * 8), 256, 0, st>>>((const float2*)op->x_ws, (float2*)op->x_ws, N, op->scal_ws);
+        else pk::normalise_kernel<double><<<grid_for(N, 256, 148 * 8), 256, 0, st>>>((const double2*)op->x_ws, (double2*)op->x_ws, N, op->scal_ws);
+        op->launches++;
+        CK(cudaGetLastError());
+        return PURIFY_OK;
+    };
+    // start vector: the caller's, or all ones
+    if (x0_dev) {
+        CK(cudaMemcpyAsync(op->x_ws, x0_dev, xb, cudaMemcpyDeviceToDevice, st));
+    } else {
+        std::vector<unsigned char> ones(xb);
+        if (f32) { float2* p = (float2*)ones.data(); for (long long i = 0; i < N; ++i) p[i] = make_float2(1.f, 0.f); }
+        else { double2* p = (double2*)ones.data(); for (long long i = 0; i < N; ++i) p[i] = make_double2(1.0, 0.0); }
+        CK(cudaMemcpyAsync(op->x_ws, ones.data(), xb, cudaMemcpyHostToDevice, st));
+        CK(cudaStreamSynchronize(st));
+    }
+    double lambda = 0.0, prev = 0.0, n2 = 0.0;
+    int it = 0;
+    RUN(norm2(op->x_ws, &n2));
+    if (!(n2 > 0.0)) return fail(PURIFY_ERR_INVALID_ARG, "power method: the start vector is zero or not finite");
+    for (it = 1; it <= max_iter; ++it) {
+        RUN(normalise());                               // ||x|| = 1
+        RUN(degrid_impl(op, op->x_ws, op->y_ws, false, st));
+        RUN(grid_impl(op, op->y_ws, op->x_ws, false, st));       // x <- Phi^dagger Phi x
+        RUN(norm2(op->x_ws, &n2));
+        prev = lambda;
+        lambda = sqrt(n2);                              // ||Phi^dagger Phi x|| with ||x|| = 1 -> largest eigenvalue
+        if (!(lambda > 0.0) || (it > 1 && fabs(lambda - prev) <= rel_tol * lambda)) break;
+    }
+    if (it > max_iter) it = max_iter;
+    *lambda_out = lambda;
+    if (iters_out) *iters_out = it;
     return PURIFY_OK;
 }
 

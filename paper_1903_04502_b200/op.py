@@ -25,7 +25,7 @@ SYMBOLS = (
     "purify_degrid_native", "purify_grid_native", "purify_permute_to_native",
     "purify_permute_from_native", "purify_degrid_host", "purify_grid_host", "purify_normal_host",
     "purify_stage_fourier_grid", "purify_stage_gridded", "purify_stage_times_ms",
-    "purify_last_launch_count", "purify_strerror", "purify_last_error", "purify_version",
+    "purify_last_launch_count", "purify_strerror", "purify_last_error", "purify_version", "purify_op_norm",
 )
 
 
@@ -72,6 +72,8 @@ def load_library():
                  "purify_grid_host", "purify_normal_host", "purify_stage_fourier_grid", "purify_stage_gridded"):
         getattr(L, name).argtypes = [vp, vp, vp, vp]
         getattr(L, name).restype = ip
+    L.purify_op_norm.argtypes = [vp, vp, ip, C.c_double, C.POINTER(C.c_double), C.POINTER(ip), vp]
+    L.purify_op_norm.restype = ip
     L.purify_stage_times_ms.argtypes = [vp, C.POINTER(C.c_float)]
     L.purify_last_launch_count.argtypes = [vp]
     L.purify_strerror.argtypes = [ip]
@@ -242,6 +244,16 @@ class PurifyOp:
         out = self._new_x("cpu").pin_memory() if out is None else out
         _check(self._L.purify_normal_host(self._h, self._x(x), self._x(out, "out"), _stream()), "purify_normal_host")
         return out
+
+    # -- f2: operator norm (largest eigenvalue of Phi^dagger Phi) by the power method
+    def norm(self, x0=None, max_iter: int = 100, rel_tol: float = 1e-6):
+        """Returns (lambda, iterations).  x0: n x n complex start vector on the device, or None for all ones."""
+        lam, its = C.c_double(0.0), C.c_int(0)
+        if x0 is not None:
+            self._dev(x0)
+        _check(self._L.purify_op_norm(self._h, self._x(x0, "x0") if x0 is not None else None, int(max_iter),
+                                      float(rel_tol), C.byref(lam), C.byref(its), _stream()), "purify_op_norm")
+        return float(lam.value), int(its.value)
 
     # -- single stages in the mathematical layout (tests)
     def stage_fourier_grid(self, x):

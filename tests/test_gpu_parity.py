@@ -288,3 +288,30 @@ def test_hot_cells_and_layer_straddling_batches():
     info = run_all_checks(x, uv, w, J, "c64")
     assert info["layout"] == 1
     run_all_checks(x, uv, w, J, "c128")
+
+
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+def test_operator_norm_power_method(dtype):
+    """f2: purify_op_norm against the oracle's power method, same start vector, same fixed number of
+    iterations (rel_tol = 0), and the stopping rule with a tolerance; also the all-ones default start."""
+    cfg, x, uv, w = synth.make_problem(1, M=4000)
+    w = synth.rng_for(11, synth.STREAM_W).uniform(0.5, 1.5, size=len(uv))
+    x0 = synth.random_complex((cfg.n, cfg.n), seed=21, dtype=dtype)
+    _, uvc, wc = cast_problem(x, uv, w, dtype)
+    op = make_op(cfg.n, cfg.J, uvc, wc, dtype)
+    tol = 1e-5 if dtype == "c64" else 1e-11
+    for iters in (1, 7):
+        lam_ref, _ = oracle.power_method(x0, uvc, wc, cfg.n, cfg.J, max_iter=iters, rel_tol=0.0, idx_prec=idx_prec(dtype))
+        lam, its = op.norm(dev(x0), max_iter=iters, rel_tol=0.0)
+        assert its == iters and abs(lam - lam_ref) <= tol * lam_ref, (iters, lam, lam_ref)
+    lam_ref, its_ref = oracle.power_method(None, uvc, wc, cfg.n, cfg.J, max_iter=200, rel_tol=1e-4, idx_prec=idx_prec(dtype))
+    lam, its = op.norm(None, max_iter=200, rel_tol=1e-4)
+    assert abs(its - its_ref) <= 1 and abs(lam - lam_ref) <= 2e-4 * lam_ref
+    # Rayleigh check with the operator itself: ||Phi^dagger Phi x|| <= lambda ||x|| (up to the convergence gap)
+    xr = synth.random_complex((cfg.n, cfg.n), seed=22, dtype=dtype)
+    lam_conv, _ = op.norm(dev(x0), max_iter=300, rel_tol=1e-7)
+    z = host(op.normal(dev(xr)))
+    assert np.linalg.norm(z) <= lam_conv * np.linalg.norm(xr) * (1 + 1e-3)
+    with pytest.raises(Exception):
+        op.norm(dev(np.zeros((cfg.n, cfg.n), dtype=synth.complex_dtype(dtype))), max_iter=3)
+    op.close()

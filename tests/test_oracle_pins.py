@@ -325,3 +325,29 @@ def test_table_index_precision_flag():
     for c in range(1233, 1237):
         assert oracle.kernel_weight(float(u32), c, J, "table", R, 32) == \
             oracle.kernel_weight(float(u32), c, J, "table", R, 64)
+
+
+def test_power_method_vs_dense_eigensolver():
+    """f2: the oracle's power method against numpy's dense eigen-solver on a tiny operator whose
+    matrix is assembled column by column (Phi applied to the n^2 basis images)."""
+    n, J, M = 8, 4, 60
+    rng = synth.rng_for(31, synth.STREAM_UV)
+    uv = rng.uniform(-n + 0.01, n - 0.01, size=(M, 2))
+    w = rng.uniform(0.5, 1.5, size=M)
+    Phi = np.empty((M, n * n), dtype=np.complex128)
+    for p in range(n * n):
+        e = np.zeros(n * n, dtype=np.complex128)
+        e[p] = 1.0
+        Phi[:, p] = oracle.degrid(e.reshape(n, n), uv, w, J)
+    lam_true = float(np.linalg.eigvalsh(Phi.conj().T @ Phi)[-1])
+    assert abs(np.linalg.norm(Phi, 2) ** 2 - lam_true) <= 1e-10 * lam_true
+    x0 = synth.random_complex((n, n), seed=3)
+    lam, its = oracle.power_method(x0, uv, w, n, J, max_iter=3000, rel_tol=1e-13)
+    assert abs(lam - lam_true) <= 1e-7 * lam_true, (lam, lam_true, its)
+    # the iterates increase monotonically towards the eigenvalue (Phi^dagger Phi is positive semi-definite)
+    lam5, _ = oracle.power_method(x0, uv, w, n, J, max_iter=5, rel_tol=0.0)
+    lam50, _ = oracle.power_method(x0, uv, w, n, J, max_iter=50, rel_tol=0.0)
+    assert lam5 <= lam50 * (1 + 1e-12) <= lam_true * (1 + 1e-9)
+    # scaling: Phi -> 2 Phi (weights doubled) multiplies the eigenvalue by 4
+    lam2, _ = oracle.power_method(x0, uv, 2 * w, n, J, max_iter=3000, rel_tol=1e-13)
+    assert abs(lam2 - 4 * lam_true) <= 1e-6 * lam_true
