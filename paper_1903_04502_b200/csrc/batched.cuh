@@ -45,9 +45,12 @@ constexpr int REC_FLOATS = 96, REC_BYTES = 384;
 #ifndef PURIFY_XVG
 #define PURIFY_XVG 1
 #endif
+#ifndef PURIFY_XVG4
+#define PURIFY_XVG4 1
+#endif
 // visibilities per inner-loop trip (statement-interleaved dependency graphs): degridding gains from 2 (0.73 ->
 // 0.69 ms at config 4, 160 registers, 3 CTAs / SM); gridding loses (its flush phases want the 4th CTA)
-constexpr int XVD = PURIFY_XVD, XVG = PURIFY_XVG;         // per-iteration record: uv[32] | w[32]
+constexpr int XVD = PURIFY_XVD, XVG6 = PURIFY_XVG, XVG4 = PURIFY_XVG4;         // per-iteration record: uv[32] | w[32]
 
 template <int J> struct XCfg {
     static constexpr int XOFF = (J / 2 - 1) & 1;        // makes the box's first column even (TMA: 16-byte aligned)
@@ -667,10 +670,11 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
 // 8-byte reduction per non-zero cell (RED.ADD.F32x2; halos of neighbouring bands and the items of
 // one band meet there).
 template <int J, int DEG, int MODE, int CH, int S>
-__global__ void __launch_bounds__(XCfg<J>::THREADS, J <= 6 ? (XVG == 1 ? 4 : 3) : 1)
+__global__ void __launch_bounds__(XCfg<J>::THREADS, J <= 6 ? 4 : 1)
 grid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, const float2* __restrict__ y) {
     typedef XCfg<J> Cfg;
     typedef RingCfg<CH, true> R;
+    constexpr int XVG = J == 4 ? XVG4 : XVG6;            // visibilities per trip
     typedef XSmem<J, CH, S, true> SM;
     constexpr int BOXW = Cfg::BOXW, BOXH = Cfg::BOXH, XOFF = Cfg::XOFF;
     extern __shared__ __align__(128) unsigned char smem_raw[];
