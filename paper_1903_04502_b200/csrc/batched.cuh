@@ -354,7 +354,8 @@ __device__ __forceinline__ float2 dup2(float a) { return make_float2(a, a); }
 // c_j = cell - J/2 + 1 + j.  ANALYTIC: t = (u - cell) - 1/2 per axis, the even / odd Horner chains of
 // the two axes run as one packed chain.  TABLE: T[floor(|u - c_j| R + 1/2)], one IEEE op per step.
 template <int J, int DEG, int MODE>
-__device__ __forceinline__ void x_weights(float2 uv, float2 cellf, int cx, int cy, const XParams& p, float2 (&g)[J]) {
+__device__ __forceinline__ void x_weights(float2 uv, float2 cellf, int cx, int cy, const XParams& p, const float* tab,
+                                          float2 (&g)[J]) {
     if (MODE == 0) {
         constexpr int NE = DEG / 2 + 1, NO = (DEG + 1) / 2;
         const float2 t = add2(add2(uv, make_float2(-cellf.x, -cellf.y)), make_float2(-0.5f, -0.5f));
@@ -376,8 +377,9 @@ __device__ __forceinline__ void x_weights(float2 uv, float2 cellf, int cx, int c
             const float dx = __fsub_rn(uv.x, (float)ox), dy = __fsub_rn(uv.y, (float)oy);
             const int ix = (int)floorf(__fadd_rn(__fmul_rn(fabsf(dx), p.table_R), 0.5f));
             const int iy = (int)floorf(__fadd_rn(__fmul_rn(fabsf(dy), p.table_R), 0.5f));
-            g[j].x = ix < p.table_len ? __ldg(p.table + ix) : 0.f;
-            g[j].y = iy < p.table_len ? __ldg(p.table + iy) : 0.f;
+            // MODE 1: table in global memory (read through L1); MODE 2: the CTA's copy in shared memory
+            g[j].x = ix < p.table_len ? (MODE == 2 ? tab[ix] : __ldg(tab + ix)) : 0.f;
+            g[j].y = iy < p.table_len ? (MODE == 2 ? tab[iy] : __ldg(tab + iy)) : 0.f;
         }
     }
 }
@@ -386,7 +388,7 @@ __device__ __forceinline__ void x_weights(float2 uv, float2 cellf, int cx, int c
 // graphs advance together (ANALYTIC; TABLE evaluates visibility by visibility).
 template <int J, int DEG, int MODE, int V>
 __device__ __forceinline__ void x_weights_v(const float2 (&uv)[V], float2 cellf, int cx, int cy, const XParams& p,
-                                            float2 (&g)[V][J]) {
+                                            const float* tab, float2 (&g)[V][J]) {
     if (MODE == 0) {
         constexpr int NE = DEG / 2 + 1, NO = (DEG + 1) / 2;
         float2 t[V], t2[V], nt[V];
@@ -414,7 +416,7 @@ __device__ __forceinline__ void x_weights_v(const float2 (&uv)[V], float2 cellf,
         }
     } else {
 #pragma unroll
-        for (int v = 0; v < V; ++v) x_weights<J, DEG, MODE>(uv[v], cellf, cx, cy, p, g[v]);
+        for (int v = 0; v < V; ++v) x_weights<J, DEG, MODE>(uv[v], cellf, cx, cy, p, tab, g[v]);
     }
 }
 
@@ -422,9 +424,9 @@ __device__ __forceinline__ void x_weights_v(const float2 (&uv)[V], float2 cellf,
 // V J instructions away), two column chains.
 template <int J, int DEG, int MODE, int V>
 __device__ __forceinline__ void x_degrid_vis(const float2 (&uv)[V], const float (&w)[V], float2 cellf, int cx, int cy,
-                                             const XParams& p, const float2 (&B)[J][J], float2 (&out)[V]) {
+                                             const XParams& p, const float* tab, const float2 (&B)[J][J], float2 (&out)[V]) {
     float2 g[V][J];
-    x_weights_v<J, DEG, MODE, V>(uv, cellf, cx, cy, p, g);
+    x_weights_v<J, DEG, MODE, V>(uv, cellf, cx, cy, p, tab, g);
     float2 r[V][J];
 #pragma unroll
     for (int a = 0; a < J; ++a)
@@ -453,9 +455,9 @@ __device__ __forceinline__ void x_degrid_vis(const float2 (&uv)[V], const float 
 // a4 arithmetic for V visibilities of one cell: A[a][c] += g_x[c] (g_y[a] w y), visibility by visibility per tap
 template <int J, int DEG, int MODE, int V>
 __device__ __forceinline__ void x_grid_vis(const float2 (&uv)[V], const float (&w)[V], const float2 (&yv)[V], float2 cellf,
-                                           int cx, int cy, const XParams& p, float2 (&A)[J][J]) {
+                                           int cx, int cy, const XParams& p, const float* tab, float2 (&A)[J][J]) {
     float2 g[V][J];
-    x_weights_v<J, DEG, MODE, V>(uv, cellf, cx, cy, p, g);
+    x_weights_v<J, DEG, MODE, V>(uv, cellf, cx, cy, p, tab, g);
     float2 z[V];
 #pragma unroll
     for (int v = 0; v < V; ++v) z[v] = mul2(dup2(w[v]), yv[v]);
@@ -503,10 +505,13 @@ template <int CH, bool WITH_Y> struct RingCfg {
     static constexpr int STAGE = REC + Y;
 };
 
-template <int J, int CH, int S, bool WITH_Y> struct XSmem {
+// warps per CTA: 4; 8 for the shared-memory-table kernels (MODE 2), so that one copy of the table serves more warps
+__host__ __device__ constexpr int x_warps(int MODE) { return MODE == 2 ? 8 : 4; }
+
+template <int J, int CH, int S, bool WITH_Y, int NW = 4> struct XSmem {
     static constexpr int WARP_BYTES = XCfg<J>::REGION_BYTES + S * RingCfg<CH, WITH_Y>::STAGE;
     static constexpr int BARS = S + 1;                   // per warp: the box + the ring stages
-    static constexpr size_t TOTAL = (size_t)XCfg<J>::WARPS * WARP_BYTES + XCfg<J>::WARPS * BARS * sizeof(uint64_t);
+    static constexpr size_t TOTAL = (size_t)NW * WARP_BYTES + NW * BARS * sizeof(uint64_t);   // (+ the table, MODE 2)
 };
 
 // one lane: start the copies of chunk c (iterations [c CH, c CH + n)) of the item into `stage`.
@@ -530,18 +535,26 @@ __device__ __forceinline__ void ring_issue(unsigned char* ring, uint64_t* rbar, 
 // per batch every lane loads its cell's J x J patch into registers and then runs its unit's
 // visibilities out of registers.  HBM per slot: uv 8 + w 4 read, y 8 written (native order).
 template <int J, int DEG, int MODE, int CH, int S>
-__global__ void __launch_bounds__(XCfg<J>::THREADS, J <= 6 ? (XVD == 1 ? 4 : (XVD == 2 ? 3 : 2)) : 1)
+__global__ void __launch_bounds__(x_warps(MODE) * 32, MODE == 2 ? 1 : (J <= 6 ? (XVD == 1 ? 4 : (XVD == 2 ? 3 : 2)) : 1))
 degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float2* __restrict__ y) {
     typedef XCfg<J> Cfg;
     typedef RingCfg<CH, false> R;
-    typedef XSmem<J, CH, S, false> SM;
+    constexpr int NW = x_warps(MODE);
+    typedef XSmem<J, CH, S, false, NW> SM;
     constexpr int BOXW = Cfg::BOXW, BOXH = Cfg::BOXH, XOFF = Cfg::XOFF;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     float2* tile = reinterpret_cast<float2*>(smem_raw + warp * SM::WARP_BYTES);
     unsigned char* ring = smem_raw + warp * SM::WARP_BYTES + Cfg::REGION_BYTES;
-    uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + Cfg::WARPS * SM::WARP_BYTES) + warp * SM::BARS;
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + NW * SM::WARP_BYTES) + warp * SM::BARS;
     uint64_t* rbar = bar + 1;
+    const float* tab = p.table;
+    if (MODE == 2) {                                    // the CTA's copy of the pre-sampled table (the only CTA-wide step)
+        float* ts = reinterpret_cast<float*>(smem_raw + SM::TOTAL);
+        for (int i = threadIdx.x; i < p.table_len; i += NW * 32) ts[i] = __ldg(p.table + i);
+        __syncthreads();
+        tab = ts;
+    }
     if (lane == 0) {
         for (int i = 0; i < SM::BARS; ++i) mbar_init(bar + i, 1);
         fence_barrier_init();
@@ -631,7 +644,7 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
                         wk[v] = rp[v * REC_FLOATS + 64];
                     }
                     rp += XVD * REC_FLOATS;
-                    x_degrid_vis<J, DEG, MODE, XVD>(uvk, wk, cellf, cx, cy, p, B, o);
+                    x_degrid_vis<J, DEG, MODE, XVD>(uvk, wk, cellf, cx, cy, p, tab, B, o);
 #pragma unroll
                     for (int v = 0; v < XVD; ++v) yout[v * 32] = o[v];
                     yout += XVD * 32;
@@ -641,7 +654,7 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
                     const float w1[1] = {rp[64]};
                     float2 o1[1];
                     rp += REC_FLOATS;
-                    x_degrid_vis<J, DEG, MODE, 1>(uv1, w1, cellf, cx, cy, p, B, o1);
+                    x_degrid_vis<J, DEG, MODE, 1>(uv1, w1, cellf, cx, cy, p, tab, B, o1);
                     *yout = o1[0];
                     yout += 32;
                 }
@@ -670,19 +683,27 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
 // 8-byte reduction per non-zero cell (RED.ADD.F32x2; halos of neighbouring bands and the items of
 // one band meet there).
 template <int J, int DEG, int MODE, int CH, int S>
-__global__ void __launch_bounds__(XCfg<J>::THREADS, J <= 6 ? 4 : 1)
+__global__ void __launch_bounds__(x_warps(MODE) * 32, MODE == 2 ? 1 : (J <= 6 ? 4 : 1))
 grid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, const float2* __restrict__ y) {
     typedef XCfg<J> Cfg;
     typedef RingCfg<CH, true> R;
     constexpr int XVG = J == 4 ? XVG4 : XVG6;            // visibilities per trip
-    typedef XSmem<J, CH, S, true> SM;
+    constexpr int NW = x_warps(MODE);
+    typedef XSmem<J, CH, S, true, NW> SM;
     constexpr int BOXW = Cfg::BOXW, BOXH = Cfg::BOXH, XOFF = Cfg::XOFF;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     float2* tile = reinterpret_cast<float2*>(smem_raw + warp * SM::WARP_BYTES);
     unsigned char* ring = smem_raw + warp * SM::WARP_BYTES + Cfg::REGION_BYTES;
-    uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + Cfg::WARPS * SM::WARP_BYTES) + warp * SM::BARS;
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + NW * SM::WARP_BYTES) + warp * SM::BARS;
     uint64_t* rbar = bar + 1;
+    const float* tab = p.table;
+    if (MODE == 2) {                                    // the CTA's copy of the pre-sampled table (the only CTA-wide step)
+        float* ts = reinterpret_cast<float*>(smem_raw + SM::TOTAL);
+        for (int i = threadIdx.x; i < p.table_len; i += NW * 32) ts[i] = __ldg(p.table + i);
+        __syncthreads();
+        tab = ts;
+    }
     if (lane == 0) {
         for (int i = 0; i < SM::BARS; ++i) mbar_init(bar + i, 1);
         fence_barrier_init();
@@ -759,7 +780,7 @@ grid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, const f
                     }
                     rp += XVG * REC_FLOATS;
                     yp += XVG * 32;
-                    x_grid_vis<J, DEG, MODE, XVG>(uvk, wk, yk, cellf, cx, cy, p, A);
+                    x_grid_vis<J, DEG, MODE, XVG>(uvk, wk, yk, cellf, cx, cy, p, tab, A);
                 }
                 for (; XVG > 1 && k < seg; ++k, --live) {
                     const float2 uv1[1] = {*reinterpret_cast<const float2*>(rp + lane)};
@@ -768,7 +789,7 @@ grid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, const f
                     if (live <= 0) y1[0] = make_float2(0.f, 0.f);
                     rp += REC_FLOATS;
                     yp += 32;
-                    x_grid_vis<J, DEG, MODE, 1>(uv1, w1, y1, cellf, cx, cy, p, A);
+                    x_grid_vis<J, DEG, MODE, 1>(uv1, w1, y1, cellf, cx, cy, p, tab, A);
                 }
                 i += seg;
                 rem -= seg;

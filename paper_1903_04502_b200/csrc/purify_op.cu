@@ -236,53 +236,59 @@ template <typename Kern> int x_grid_size(Kern kern, int threads, size_t smem, in
 #define PURIFY_X_SG 2
 #endif
 constexpr int X_CH_DEGRID = PURIFY_X_CHD, X_S_DEGRID = PURIFY_X_SD, X_CH_GRID = PURIFY_X_CHG, X_S_GRID = PURIFY_X_SG;
-// TABLE mode: the table (R J/2 + 2 floats, 32 KB at R = 4096, J = 4) must stay resident in L1, which is what
-// the shared-memory carve-out leaves over.  Measured at config 5: grid 26.8 ms with a (4, 2) ring (table
-// evicted, every lookup an L2 access), 4.4 ms with (3, 2).  Smaller rings for the table kernels.
+// TABLE mode.  A table of up to 64 KB (R J/2 + 2 floats; 32 KB at R = 4096, J = 4) is copied into shared memory by
+// every CTA (MODE 2, 8 warps per CTA): 32 lanes looking up unrelated entries cost ~3.5 shared-memory wavefronts per
+// lookup, against many more L1 tag look-ups when the table sits in global memory.  Larger tables (the paper's
+// R = 2e5) stay in global memory (MODE 1) with small rings, so that L1 keeps as much of the table as it can
+// (measured at config 5 before MODE 2 existed: grid 26.8 ms with a (4, 2) ring - table evicted from L1 - and
+// 4.4 ms with (3, 2)).
 constexpr int X_CH_DEGRID_T = 4, X_S_DEGRID_T = 2, X_CH_GRID_T = 3, X_S_GRID_T = 2;
+constexpr size_t X_TABLE_SMEM_MAX = 64 * 1024;
 
-template <int J, int DEG> int launch_degrid_x_t(purify_op* op, void* y, cudaStream_t st) {
-    typedef pk::XCfg<J> Cfg;
-    if (op->n_items == 0) return PURIFY_OK;
-    size_t smem = pk::XSmem<J, X_CH_DEGRID, X_S_DEGRID, false>::TOTAL;
+template <int J, int DEG, int MODE, int CH, int S>
+int launch_degrid_x_m(purify_op* op, void* y, size_t extra_smem, cudaStream_t st) {
+    constexpr int NW = pk::x_warps(MODE);
+    const size_t smem = pk::XSmem<J, CH, S, false, NW>::TOTAL + extra_smem;
     const pk::XParams p = make_xparams(op, false);
     CK(cudaMemsetAsync(op->x_counter, 0, sizeof(unsigned), st));
     int g = 0, rc;
-    if (op->mode == PURIFY_KERNEL_TABLE) {
-        smem = pk::XSmem<J, X_CH_DEGRID_T, X_S_DEGRID_T, false>::TOTAL;
-        auto kern = pk::degrid_x_kernel<J, DEG, 1, X_CH_DEGRID_T, X_S_DEGRID_T>;
-        if ((rc = x_grid_size(kern, Cfg::THREADS, smem, op->n_items, Cfg::WARPS, &g))) return rc;
-        kern<<<g, Cfg::THREADS, smem, st>>>(op->tmap_x, p, (float2*)y);
-    } else {
-        auto kern = pk::degrid_x_kernel<J, DEG, 0, X_CH_DEGRID, X_S_DEGRID>;
-        if ((rc = x_grid_size(kern, Cfg::THREADS, smem, op->n_items, Cfg::WARPS, &g))) return rc;
-        kern<<<g, Cfg::THREADS, smem, st>>>(op->tmap_x, p, (float2*)y);
-    }
+    auto kern = pk::degrid_x_kernel<J, DEG, MODE, CH, S>;
+    if ((rc = x_grid_size(kern, NW * 32, smem, op->n_items, NW, &g))) return rc;
+    kern<<<g, NW * 32, smem, st>>>(op->tmap_x, p, (float2*)y);
     op->launches++;
     CK(cudaGetLastError());
     return PURIFY_OK;
 }
 
-template <int J, int DEG> int launch_grid_x_t(purify_op* op, const void* y, cudaStream_t st) {
-    typedef pk::XCfg<J> Cfg;
-    if (op->n_items == 0) return PURIFY_OK;
-    size_t smem = pk::XSmem<J, X_CH_GRID, X_S_GRID, true>::TOTAL;
+template <int J, int DEG, int MODE, int CH, int S>
+int launch_grid_x_m(purify_op* op, const void* y, size_t extra_smem, cudaStream_t st) {
+    constexpr int NW = pk::x_warps(MODE);
+    const size_t smem = pk::XSmem<J, CH, S, true, NW>::TOTAL + extra_smem;
     const pk::XParams p = make_xparams(op, false);
     CK(cudaMemsetAsync(op->x_counter, 0, sizeof(unsigned), st));
     int g = 0, rc;
-    if (op->mode == PURIFY_KERNEL_TABLE) {
-        smem = pk::XSmem<J, X_CH_GRID_T, X_S_GRID_T, true>::TOTAL;
-        auto kern = pk::grid_x_kernel<J, DEG, 1, X_CH_GRID_T, X_S_GRID_T>;
-        if ((rc = x_grid_size(kern, Cfg::THREADS, smem, op->n_items, Cfg::WARPS, &g))) return rc;
-        kern<<<g, Cfg::THREADS, smem, st>>>(op->tmap_x, p, (const float2*)y);
-    } else {
-        auto kern = pk::grid_x_kernel<J, DEG, 0, X_CH_GRID, X_S_GRID>;
-        if ((rc = x_grid_size(kern, Cfg::THREADS, smem, op->n_items, Cfg::WARPS, &g))) return rc;
-        kern<<<g, Cfg::THREADS, smem, st>>>(op->tmap_x, p, (const float2*)y);
-    }
+    auto kern = pk::grid_x_kernel<J, DEG, MODE, CH, S>;
+    if ((rc = x_grid_size(kern, NW * 32, smem, op->n_items, NW, &g))) return rc;
+    kern<<<g, NW * 32, smem, st>>>(op->tmap_x, p, (const float2*)y);
     op->launches++;
     CK(cudaGetLastError());
     return PURIFY_OK;
+}
+
+template <int J, int DEG> int launch_degrid_x_t(purify_op* op, void* y, cudaStream_t st) {
+    if (op->n_items == 0) return PURIFY_OK;
+    const size_t tb = sizeof(float) * (size_t)op->table_len;
+    if (op->mode != PURIFY_KERNEL_TABLE) return launch_degrid_x_m<J, DEG, 0, X_CH_DEGRID, X_S_DEGRID>(op, y, 0, st);
+    if (tb <= X_TABLE_SMEM_MAX) return launch_degrid_x_m<J, DEG, 2, X_CH_DEGRID_T, X_S_DEGRID_T>(op, y, tb, st);
+    return launch_degrid_x_m<J, DEG, 1, X_CH_DEGRID_T, X_S_DEGRID_T>(op, y, 0, st);
+}
+
+template <int J, int DEG> int launch_grid_x_t(purify_op* op, const void* y, cudaStream_t st) {
+    if (op->n_items == 0) return PURIFY_OK;
+    const size_t tb = sizeof(float) * (size_t)op->table_len;
+    if (op->mode != PURIFY_KERNEL_TABLE) return launch_grid_x_m<J, DEG, 0, X_CH_GRID, X_S_GRID>(op, y, 0, st);
+    if (tb <= X_TABLE_SMEM_MAX) return launch_grid_x_m<J, DEG, 2, X_CH_GRID_T, X_S_GRID_T>(op, y, tb, st);
+    return launch_grid_x_m<J, DEG, 1, X_CH_GRID_T, X_S_GRID_T>(op, y, 0, st);
 }
 
 int launch_degrid(purify_op* op, void* y, bool caller_order, cudaStream_t st) {
