@@ -145,6 +145,17 @@ int purify_normal_host(purify_op *op, const void *x_in_host, void *x_out_host, v
 int purify_op_norm(purify_op *op, const void *x0_dev, int max_iter, double rel_tol, double *lambda_out, int *iters_out,
                    void *cuda_stream);
 
+/* f1: the data-fidelity half of one ADMM iteration around the operator - Algorithm 1 lines 3-6
+ * with the l2-ball projection of Eq. (23):
+ *     v = Phi x;   r = P_B(v + s), B = { z : ||z - y||_2 <= epsilon };   s <- s + varrho (v - r);
+ *     g = Phi^dagger (v - r + s)          (the caller then forms x~ = x - rho g, line 6).
+ * y_native_dev (measurements) and s_native_dev (dual variable, updated in place) are NATIVE-order vectors of M_native
+ * entries (bring the data there once with purify_permute_to_native; padding entries are ignored and s is written as 0
+ * there).  g_dev: n*n complex, device.  resid_norm_out: HOST pointer that receives ||v + s_old - y||_2 (may be NULL;
+ * if given the call synchronises the stream).  epsilon >= 0. */
+int purify_admm_fidelity_step(purify_op *op, const void *x_dev, const void *y_native_dev, void *s_native_dev,
+                              double epsilon, double varrho, void *g_dev, double *resid_norm_out, void *cuda_stream);
+
 /* Stage access for tests (device pointers): the K x K Fourier grid workspace in the library's
  * internal layout is NOT exposed; these run single stages into caller buffers in the mathematical
  * layout B[ky*K + kx], ky, kx in [0, K) (DC at index 0), so they can be compared with the oracle. */

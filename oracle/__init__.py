@@ -225,3 +225,21 @@ def power_method(x0, uv, w, n, J, max_iter=100, rel_tol=1e-6, mode="analytic", R
         if not lam > 0.0 or (it > 1 and abs(lam - prev) <= rel_tol * lam):
             break
     return lam, it
+
+
+def admm_fidelity_step(x, y, s, uv, w, n, J, epsilon, varrho, mode="analytic", R=4096, idx_prec=64):
+    """f1: Algorithm 1 lines 3-6 in the paper's order, caller-order vectors:
+        v = Phi x                                    (line 3)
+        r = P_B(v + s), ball of radius epsilon around y:  r = v + s if ||v + s - y|| <= epsilon,
+                                                          else y + epsilon (v + s - y)/||v + s - y||   (line 4, Eq. 23)
+        s_new = s + varrho (v - r)                   (line 5)
+        g = Phi^dagger (v - r + s_new)               (line 6; the caller forms x~ = x - rho g)
+    Returns (g, s_new, r, ||v + s - y||)."""
+    y, s = _c128(y), _c128(s)
+    v = degrid(x, uv, w, J, mode, R, idx_prec)
+    d = v + s - y
+    nrm = float(np.linalg.norm(d))
+    r = v + s if nrm <= epsilon else y + d * (epsilon / nrm)
+    s_new = s + varrho * (v - r)
+    g = grid(v - r + s_new, uv, w, n, J, mode, R, idx_prec)
+    return g, s_new, r, nrm

@@ -339,4 +339,59 @@ __global__ void __launch_bounds__(256) normalise_kernel(const typename Cplx<R>::
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// f1: the data-fidelity half of one ADMM iteration around the operator (Algorithm 1 lines 3-6,
+// PAPER.md:224-231; Eq. 23), on native-order vectors.  With d = v + s - y and
+// alpha = 1 if ||d|| <= eps else eps / ||d||:   r = y + alpha d  (projection onto the l2 ball of radius eps around y),
+// v - r = (1 - alpha) d - s,   s_new = s + varrho (v - r),   z = v - r + s_new  (what Phi^dagger is applied to).
+// Padding entries of the complex64 layout (perm = 0xFFFFFFFF) count as 0 and are written as 0.
+template <typename R>
+__global__ void __launch_bounds__(256) admm_norm2_kernel(const typename Cplx<R>::type* __restrict__ v,
+                                                         const typename Cplx<R>::type* __restrict__ s,
+                                                         const typename Cplx<R>::type* __restrict__ y,
+                                                         const unsigned* __restrict__ perm, long long count,
+                                                         double* __restrict__ out) {
+    double acc = 0.0;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < count; i += (long long)gridDim.x * blockDim.x) {
+        if (perm && perm[i] == 0xFFFFFFFFu) continue;
+        const typename Cplx<R>::type a = v[i], b = s[i], c = y[i];
+        const R dx = (a.x + b.x) - c.x, dy = (a.y + b.y) - c.y;
+        acc += (double)dx * (double)dx + (double)dy * (double)dy;
+    }
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);
+    __shared__ double part[8];
+    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < 8; ++w) t += part[w];
+        atomicAdd(out, t);
+    }
+}
+
+// alpha of the projection from the device-resident ||d||^2 (the same expression in every kernel that needs it)
+__device__ __forceinline__ double admm_alpha(double norm2, double eps) {
+    const double nrm = sqrt(norm2);
+    return nrm <= eps ? 1.0 : eps / nrm;
+}
+
+template <typename R>
+__global__ void __launch_bounds__(256) admm_update_kernel(const typename Cplx<R>::type* __restrict__ v,
+                                                          typename Cplx<R>::type* __restrict__ s,      // in / out
+                                                          const typename Cplx<R>::type* __restrict__ y,
+                                                          const unsigned* __restrict__ perm, long long count,
+                                                          const double* __restrict__ norm2, double eps, double varrho,
+                                                          typename Cplx<R>::type* __restrict__ z) {
+    const R oma = (R)(1.0 - admm_alpha(*norm2, eps)), rho = (R)varrho;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < count; i += (long long)gridDim.x * blockDim.x) {
+        if (perm && perm[i] == 0xFFFFFFFFu) { s[i] = mk2<R>((R)0, (R)0); z[i] = mk2<R>((R)0, (R)0); continue; }
+        const typename Cplx<R>::type a = v[i], b = s[i], c = y[i];
+        const R dx = (a.x + b.x) - c.x, dy = (a.y + b.y) - c.y;
+        const R vrx = oma * dx - b.x, vry = oma * dy - b.y;          // v - r
+        const R sx = b.x + rho * vrx, sy = b.y + rho * vry;          // s_new
+        s[i] = mk2<R>(sx, sy);
+        z[i] = mk2<R>(vrx + sx, vry + sy);
+    }
+}
+
 }  // namespace pk

@@ -300,13 +300,7 @@ int launch_degrid(purify_op* op, void* y, bool caller_order, cudaStream_t st) {
             default: return launch_degrid_x_t<8, deg_c64(8)>(op, y, st);
         }
     }
-    if (op->dtype == PURIFY_C64) {
-        switch (op->J) {
-            case 4: return launch_degrid_t<float, 4, deg_c64(4)>(op, y, caller_order, st);
-            case 6: return launch_degrid_t<float, 6, deg_c64(6)>(op, y, caller_order, st);
-            default: return launch_degrid_t<float, 8, deg_c64(8)>(op, y, caller_order, st);
-        }
-    }
+    // complex64 always uses the batched layout above; the tile-sorted kernels below serve complex128
     switch (op->J) {
         case 4: return launch_degrid_t<double, 4, deg_c128(4)>(op, y, caller_order, st);
         case 6: return launch_degrid_t<double, 6, deg_c128(6)>(op, y, caller_order, st);
@@ -325,13 +319,6 @@ int launch_grid(purify_op* op, const void* y, bool caller_order, cudaStream_t st
             case 4: return launch_grid_x_t<4, deg_c64(4)>(op, y, st);
             case 6: return launch_grid_x_t<6, deg_c64(6)>(op, y, st);
             default: return launch_grid_x_t<8, deg_c64(8)>(op, y, st);
-        }
-    }
-    if (op->dtype == PURIFY_C64) {
-        switch (op->J) {
-            case 4: return launch_grid_t<float, 4, deg_c64(4)>(op, y, caller_order, st);
-            case 6: return launch_grid_t<float, 6, deg_c64(6)>(op, y, caller_order, st);
-            default: return launch_grid_t<float, 8, deg_c64(8)>(op, y, caller_order, st);
         }
     }
     switch (op->J) {
@@ -1054,6 +1041,55 @@ int purify_op_norm(purify_op* op, const void* x0_dev, int max_iter, double rel_t
     if (it > max_iter) it = max_iter;
     *lambda_out = lambda;
     if (iters_out) *iters_out = it;
+    return PURIFY_OK;
+}
+
+// ---- f1: data-fidelity half of one ADMM iteration (Algorithm 1 lines 3-6), native-order vectors
+int purify_admm_fidelity_step(purify_op* op, const void* x_dev, const void* y_native_dev, void* s_native_dev, double epsilon,
+                              double varrho, void* g_dev, double* resid_norm_out, void* cuda_stream) {
+    NEED_OP(op); NEED_PTR(x_dev, "x"); NEED_PTR(g_dev, "g");
+    if (op->M > 0) { NEED_PTR(y_native_dev, "y_native"); NEED_PTR(s_native_dev, "s_native"); }
+    if (!(epsilon >= 0.0)) return fail(PURIFY_ERR_INVALID_ARG, "epsilon must be >= 0");
+    begin_call(op);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const long long Mn = op->M_native;
+    RUN(ensure_ws(op, &op->y_ws, csize(op) * (size_t)Mn));
+    RUN(ensure_ws(op, &op->y_ws2, csize(op) * (size_t)(Mn > op->M ? Mn : op->M)));
+    RUN(ensure_ws(op, (void**)&op->scal_ws, sizeof(double)));
+    const unsigned* pm = op->batched ? op->perm : nullptr;     // padding mask (complex64 layout only)
+    // line 3: v = Phi x
+    RUN(degrid_impl(op, x_dev, op->y_ws, false, st));
+    // line 4: ||v + s - y||^2 (fp64 accumulation)
+    CK(cudaMemsetAsync(op->scal_ws, 0, sizeof(double), st));
+    if (Mn > 0) {
+        if (op->dtype == PURIFY_C64)
+            pk::admm_norm2_kernel<float><<<grid_for(Mn, 256, 148 * 8), 256, 0, st>>>((const float2*)op->y_ws, (const float2*)s_native_dev,
+                                                                                    (const float2*)y_native_dev, pm, Mn, op->scal_ws);
+        else
+            pk::admm_norm2_kernel<double><<<grid_for(Mn, 256, 148 * 8), 256, 0, st>>>((const double2*)op->y_ws, (const double2*)s_native_dev,
+                                                                                     (const double2*)y_native_dev, pm, Mn, op->scal_ws);
+        op->launches++;
+        CK(cudaGetLastError());
+        // lines 4-6: r, s <- s + varrho (v - r), z = v - r + s
+        if (op->dtype == PURIFY_C64)
+            pk::admm_update_kernel<float><<<grid_for(Mn, 256, 148 * 16), 256, 0, st>>>((const float2*)op->y_ws, (float2*)s_native_dev,
+                                                                                      (const float2*)y_native_dev, pm, Mn, op->scal_ws,
+                                                                                      epsilon, varrho, (float2*)op->y_ws2);
+        else
+            pk::admm_update_kernel<double><<<grid_for(Mn, 256, 148 * 16), 256, 0, st>>>((const double2*)op->y_ws, (double2*)s_native_dev,
+                                                                                       (const double2*)y_native_dev, pm, Mn, op->scal_ws,
+                                                                                       epsilon, varrho, (double2*)op->y_ws2);
+        op->launches++;
+        CK(cudaGetLastError());
+    }
+    // line 6: g = Phi^dagger (v - r + s)
+    RUN(grid_impl(op, op->y_ws2, g_dev, false, st));
+    if (resid_norm_out) {
+        double n2 = 0.0;
+        CK(cudaMemcpyAsync(&n2, op->scal_ws, sizeof(double), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        *resid_norm_out = sqrt(n2);
+    }
     return PURIFY_OK;
 }
 

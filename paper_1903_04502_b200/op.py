@@ -25,7 +25,7 @@ SYMBOLS = (
     "purify_degrid_native", "purify_grid_native", "purify_permute_to_native",
     "purify_permute_from_native", "purify_degrid_host", "purify_grid_host", "purify_normal_host",
     "purify_stage_fourier_grid", "purify_stage_gridded", "purify_stage_times_ms",
-    "purify_last_launch_count", "purify_strerror", "purify_last_error", "purify_version", "purify_op_norm",
+    "purify_last_launch_count", "purify_strerror", "purify_last_error", "purify_version", "purify_op_norm", "purify_admm_fidelity_step",
 )
 
 
@@ -74,6 +74,8 @@ def load_library():
         getattr(L, name).restype = ip
     L.purify_op_norm.argtypes = [vp, vp, ip, C.c_double, C.POINTER(C.c_double), C.POINTER(ip), vp]
     L.purify_op_norm.restype = ip
+    L.purify_admm_fidelity_step.argtypes = [vp, vp, vp, vp, C.c_double, C.c_double, vp, C.POINTER(C.c_double), vp]
+    L.purify_admm_fidelity_step.restype = ip
     L.purify_stage_times_ms.argtypes = [vp, C.POINTER(C.c_float)]
     L.purify_last_launch_count.argtypes = [vp]
     L.purify_strerror.argtypes = [ip]
@@ -254,6 +256,18 @@ class PurifyOp:
         _check(self._L.purify_op_norm(self._h, self._x(x0, "x0") if x0 is not None else None, int(max_iter),
                                       float(rel_tol), C.byref(lam), C.byref(its), _stream()), "purify_op_norm")
         return float(lam.value), int(its.value)
+
+    # -- f1: data-fidelity half of one ADMM iteration (Algorithm 1 lines 3-6), native-order y and s (s updated in place)
+    def admm_fidelity_step(self, x, y_native, s_native, epsilon: float, varrho: float, g=None, want_norm: bool = True):
+        """Returns (g, ||v + s_old - y||_2 or None) with g = Phi^dagger (v - r + s_new); s_native is updated in place."""
+        g = self._new_x() if g is None else g
+        self._dev(x, y_native, s_native, g)
+        nrm = C.c_double(0.0)
+        _check(self._L.purify_admm_fidelity_step(self._h, self._x(x), self._y(y_native, "y_native", True),
+                                                 self._y(s_native, "s_native", True), float(epsilon), float(varrho),
+                                                 self._x(g, "g"), C.byref(nrm) if want_norm else None, _stream()),
+               "purify_admm_fidelity_step")
+        return g, (float(nrm.value) if want_norm else None)
 
     # -- single stages in the mathematical layout (tests)
     def stage_fourier_grid(self, x):

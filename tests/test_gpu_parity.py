@@ -315,3 +315,34 @@ def test_operator_norm_power_method(dtype):
     with pytest.raises(Exception):
         op.norm(dev(np.zeros((cfg.n, cfg.n), dtype=synth.complex_dtype(dtype))), max_iter=3)
     op.close()
+
+
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+@pytest.mark.parametrize("case", ["outside", "inside", "eps0"])
+def test_admm_fidelity_step(dtype, case):
+    """f1 (Algorithm 1 lines 3-6): purify_admm_fidelity_step against the oracle - g, the updated dual
+    variable and the residual norm; native-order vectors, garbage in the padding entries of y and s."""
+    cfg, x, uv, w = synth.make_problem(2, M=30000, J=6)
+    x, uv, w = cast_problem(x, uv, w, dtype)
+    M = len(uv)
+    op = make_op(cfg.n, 6, uv, w, dtype)
+    y = synth.random_complex((M,), seed=51, dtype=dtype)
+    s = (synth.random_complex((M,), seed=52, dtype=dtype) * 0.25).astype(y.dtype)
+    v = oracle.degrid(x, uv, w, 6, idx_prec=idx_prec(dtype))
+    nd = float(np.linalg.norm(v + s - y))
+    eps = {"outside": 0.4 * nd, "inside": 5.0 * nd, "eps0": 0.0}[case]
+    g_ref, s_ref, _, nrm_ref = oracle.admm_fidelity_step(x, y, s, uv, w, cfg.n, 6, eps, 0.9, idx_prec=idx_prec(dtype))
+    perm = host(op.permutation())
+    valid = perm >= 0
+    y_nat = np.full(len(perm), np.nan + 1j * np.nan, dtype=y.dtype)      # padding holds NaN: must be ignored
+    s_nat = np.full(len(perm), np.nan + 1j * np.nan, dtype=y.dtype)
+    y_nat[valid], s_nat[valid] = y[perm[valid]], s[perm[valid]]
+    s_dev = dev(s_nat)
+    g, nrm = op.admm_fidelity_step(dev(x), dev(y_nat), s_dev, eps, 0.9)
+    tol = TOL[dtype]
+    assert abs(nrm - nrm_ref) <= 10 * tol * nrm_ref
+    assert rel_l2(host(g), g_ref) <= 4 * tol
+    s_out = host(s_dev)
+    assert rel_l2(s_out[valid], s_ref[perm[valid]]) <= 4 * tol
+    assert not np.any(s_out[~valid])
+    op.close()

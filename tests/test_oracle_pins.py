@@ -351,3 +351,39 @@ def test_power_method_vs_dense_eigensolver():
     # scaling: Phi -> 2 Phi (weights doubled) multiplies the eigenvalue by 4
     lam2, _ = oracle.power_method(x0, uv, 2 * w, n, J, max_iter=3000, rel_tol=1e-13)
     assert abs(lam2 - 4 * lam_true) <= 1e-6 * lam_true
+
+
+def test_admm_fidelity_step_closed_forms(tiny):
+    """f1: Algorithm 1 lines 3-6 with the projection of Eq. (23) - special cases
+    with closed forms, and the defining properties of the projection."""
+    cfg, x, uv, w = tiny
+    M = 1500
+    uv, w = uv[:M], w[:M] * 0 + synth.rng_for(5, synth.STREAM_W).uniform(0.5, 1.5, size=M)
+    y = synth.random_complex((M,), seed=41)
+    s = synth.random_complex((M,), seed=42) * 0.3
+    v = oracle.degrid(x, uv, w, cfg.J)
+    d = v + s - y
+    nd = np.linalg.norm(d)
+    # (i) inside the ball (huge epsilon): r = v + s, s_new = (1 - varrho) s, g = -varrho Phi^dagger s
+    g, s_new, r, nrm = oracle.admm_fidelity_step(x, y, s, uv, w, cfg.n, cfg.J, epsilon=10 * nd, varrho=0.9)
+    assert abs(nrm - nd) <= 1e-12 * nd
+    assert np.allclose(r, v + s, rtol=0, atol=1e-13) and np.allclose(s_new, 0.1 * s, rtol=0, atol=1e-13)
+    g_ref = -0.9 * oracle.grid(s, uv, w, cfg.n, cfg.J)
+    assert np.linalg.norm(g - g_ref) <= 1e-12 * np.linalg.norm(g_ref)
+    # (ii) epsilon = 0: r = y, s_new = s + varrho (v - y), g = Phi^dagger (v - y + s_new)
+    g, s_new, r, _ = oracle.admm_fidelity_step(x, y, s, uv, w, cfg.n, cfg.J, epsilon=0.0, varrho=0.5)
+    assert np.allclose(r, y, rtol=0, atol=1e-13) and np.allclose(s_new, s + 0.5 * (v - y), rtol=0, atol=1e-13)
+    g_ref = oracle.grid(v - y + s_new, uv, w, cfg.n, cfg.J)
+    assert np.linalg.norm(g - g_ref) <= 1e-12 * np.linalg.norm(g_ref)
+    # (iii) outside the ball: r lies ON the sphere, on the segment from y to v + s, and is the nearest point of the ball
+    eps = 0.37 * nd
+    g, s_new, r, _ = oracle.admm_fidelity_step(x, y, s, uv, w, cfg.n, cfg.J, epsilon=eps, varrho=0.9)
+    assert abs(np.linalg.norm(r - y) - eps) <= 1e-12 * eps
+    t = np.vdot(d, r - y) / np.vdot(d, d)
+    assert abs(t.imag) <= 1e-13 and abs(t.real - 0.37) <= 1e-12
+    rng = synth.rng_for(77, synth.STREAM_TEST)
+    for _ in range(20):                                   # random points of the ball are never closer to v + s
+        q = synth.random_complex((M,), seed=int(rng.integers(1 << 30)))
+        q = y + q / np.linalg.norm(q) * eps * rng.uniform(0, 1)
+        assert np.linalg.norm(q - (v + s)) >= np.linalg.norm(r - (v + s)) * (1 - 1e-12)
+    assert np.allclose(s_new, s + 0.9 * (v - r), rtol=0, atol=1e-13)
