@@ -314,6 +314,15 @@ def run_ours(args):
     norm_info = {"lambda_after_10_iterations": lam, "ms_per_iteration": (time.perf_counter() - t0) * 1e3 / max(its, 1),
                  "note": "purify_op_norm: Phi^dagger Phi + fp64 norm + scaling per iteration, host-synchronised every iteration"}
 
+    # ---- f1: Algorithm 1 lines 3-6 around the operator (fused for complex64 + analytic weights), native-order vectors
+    y_obs = op.degrid(x_dev, native=True)
+    y_obs.mul_(1.01)
+    s_dual = torch.zeros_like(y_obs)
+    ms_admm = timed(lambda: op.admm_fidelity_step(x_dev, y_obs, s_dual, 1.0, 0.9, out_dev, want_norm=False), reps)
+    admm_info = {"ms": ms_admm, "ms_minus_phi_dagger_phi": ms_admm - ms_step,
+                 "note": "purify_admm_fidelity_step: v = Phi x, l2-ball projection, dual update, Phi^dagger (v - r + s)"}
+    del y_obs, s_dual
+
     # ---- end to end through the C ABI with HOST buffers (H2D of x, D2H of the result inside)
     op.normal_host(x_pin, out_pin)
     barrier()
@@ -370,6 +379,7 @@ def run_ours(args):
                           "phi_dagger_ms": ms_phit, "phi_dagger_vis_per_s": M / (ms_phit * 1e-3),
                           "phi_caller_order_ms": ms_phi_caller, "phi_dagger_caller_order_ms": ms_phit_caller},
             "operator_norm": norm_info,
+            "admm_fidelity_step": admm_info,
             "clocks": clocks,
             "setup": {"generate_s": t_gen, "create_s": t_create, "n_items": info["n_items"],
                       "n_tiles_nonempty": info["n_tiles_nonempty"], "max_tile_count": info["max_tile_count"],

@@ -65,7 +65,8 @@ typedef struct {
                                    T[i] = g(i/R), i = 0..R*J/2+1, lookup T[floor(|d| R + 1/2)].      */
     int chunk;                  /* visibilities per work item (CTA); default 4096                    */
     int time_stages;            /* != 0: record CUDA events around each stage                        */
-    int reserved[4];
+    int reserved[4];            /* reserved[0] != 0: purify_admm_fidelity_step runs its unfused form (separate norm and
+                                   update kernels) even where the fused kernels exist; others must be 0              */
 } purify_opts;
 
 /* Facts about a handle (for tests, benches and roofline arithmetic). */
@@ -152,7 +153,10 @@ int purify_op_norm(purify_op *op, const void *x0_dev, int max_iter, double rel_t
  * y_native_dev (measurements) and s_native_dev (dual variable, updated in place) are NATIVE-order vectors of M_native
  * entries (bring the data there once with purify_permute_to_native; padding entries are ignored and s is written as 0
  * there).  g_dev: n*n complex, device.  resid_norm_out: HOST pointer that receives ||v + s_old - y||_2 (may be NULL;
- * if given the call synchronises the stream).  epsilon >= 0. */
+ * if given the call synchronises the stream).  epsilon >= 0.  PURIFY_C64 + ANALYTIC weights run fused: the norm is
+ * accumulated inside the degridding kernel and r, s_new and v - r + s_new are formed inside the gridding kernel (the
+ * vector handed to Phi^dagger is never stored); y_native and s_native must then be 16-byte aligned.  Other
+ * configurations use separate norm / update kernels. */
 int purify_admm_fidelity_step(purify_op *op, const void *x_dev, const void *y_native_dev, void *s_native_dev,
                               double epsilon, double varrho, void *g_dev, double *resid_norm_out, void *cuda_stream);
 

@@ -82,6 +82,12 @@ struct XParams {
     const float* table;
     float table_R;
     int table_len;
+    // f1 (fused ADMM data-fidelity step): dual variable s (in / out), measurements y, ||v + s - y||^2, radius, step
+    const float2* s_in;
+    const float2* yobs;
+    float2* s_out;
+    double* norm2;
+    double eps, varrho;
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -500,16 +506,18 @@ __device__ __forceinline__ void sts_v2(uint32_t a, float2 v) {
     asm volatile("st.volatile.shared.v2.f32 [%0], {%1, %2};" ::"r"(a), "f"(v.x), "f"(v.y) : "memory");
 }
 
-template <int CH, bool WITH_Y> struct RingCfg {
-    static constexpr int REC = CH * REC_BYTES, Y = WITH_Y ? CH * 256 : 0;
-    static constexpr int STAGE = REC + Y;
+// NY = number of complex64 native-order vectors streamed next to the records: 0 (degridding), 1 (gridding: y),
+// 2 (degridding + residual norm of the ADMM step: s, y), 3 (gridding of the ADMM step: v, s, y)
+template <int CH, int NY> struct RingCfg {
+    static constexpr int REC = CH * REC_BYTES, Y = CH * 256;
+    static constexpr int STAGE = REC + NY * Y;
 };
 
 // warps per CTA: 4; 8 for the shared-memory-table kernels (MODE 2), so that one copy of the table serves more warps
 __host__ __device__ constexpr int x_warps(int MODE) { return MODE == 2 ? 8 : 4; }
 
-template <int J, int CH, int S, bool WITH_Y, int NW = 4> struct XSmem {
-    static constexpr int WARP_BYTES = XCfg<J>::REGION_BYTES + S * RingCfg<CH, WITH_Y>::STAGE;
+template <int J, int CH, int S, int NY, int NW = 4> struct XSmem {
+    static constexpr int WARP_BYTES = XCfg<J>::REGION_BYTES + S * RingCfg<CH, NY>::STAGE;
     static constexpr int BARS = S + 1;                   // per warp: the box + the ring stages
     static constexpr size_t TOTAL = (size_t)NW * WARP_BYTES + NW * BARS * sizeof(uint64_t);   // (+ the table, MODE 2)
 };
@@ -517,16 +525,18 @@ template <int J, int CH, int S, bool WITH_Y, int NW = 4> struct XSmem {
 // one lane: start the copies of chunk c (iterations [c CH, c CH + n)) of the item into `stage`.
 // (No proxy fence: the stage was only READ through the generic proxy, and those reads are ordered
 // before this call by the __syncwarp() that precedes it.)
-template <int CH, bool WITH_Y>
+template <int CH, int NY>
 __device__ __forceinline__ void ring_issue(unsigned char* ring, uint64_t* rbar, int stage, const XParams& p,
-                                           const float2* y, unsigned iter0, int c, int T) {
-    typedef RingCfg<CH, WITH_Y> R;
+                                           const float2* y0, const float2* y1, const float2* y2, unsigned iter0, int c, int T) {
+    typedef RingCfg<CH, NY> R;
     const int n = min(CH, T - c * CH);
     const size_t i0 = (size_t)iter0 + (size_t)c * CH;
     unsigned char* st = ring + stage * R::STAGE;
-    mbar_expect_tx(rbar + stage, (uint32_t)(n * (REC_BYTES + (WITH_Y ? 256 : 0))));
+    mbar_expect_tx(rbar + stage, (uint32_t)(n * (REC_BYTES + NY * 256)));
     bulk_g2s(st, p.rec + i0 * REC_FLOATS, (uint32_t)(n * REC_BYTES), rbar + stage);
-    if (WITH_Y) bulk_g2s(st + R::REC, y + i0 * 32, (uint32_t)(n * 256), rbar + stage);
+    if (NY >= 1) bulk_g2s(st + R::REC, y0 + i0 * 32, (uint32_t)(n * 256), rbar + stage);
+    if (NY >= 2) bulk_g2s(st + R::REC + R::Y, y1 + i0 * 32, (uint32_t)(n * 256), rbar + stage);
+    if (NY >= 3) bulk_g2s(st + R::REC + 2 * R::Y, y2 + i0 * 32, (uint32_t)(n * 256), rbar + stage);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -534,13 +544,15 @@ __device__ __forceinline__ void ring_issue(unsigned char* ring, uint64_t* rbar, 
 // warp's private shared-memory region and the item's visibility stream runs through the warp's ring;
 // per batch every lane loads its cell's J x J patch into registers and then runs its unit's
 // visibilities out of registers.  HBM per slot: uv 8 + w 4 read, y 8 written (native order).
-template <int J, int DEG, int MODE, int CH, int S>
+// FUSE = 1 (f1): additionally streams s and y and accumulates ||v + s - y||^2 over the real slots into *p.norm2 (fp64).
+template <int J, int DEG, int MODE, int CH, int S, int FUSE = 0>
 __global__ void __launch_bounds__(x_warps(MODE) * 32, MODE == 2 ? 1 : (J <= 6 ? (XVD == 1 ? 4 : (XVD == 2 ? 3 : 2)) : 1))
 degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float2* __restrict__ y) {
     typedef XCfg<J> Cfg;
-    typedef RingCfg<CH, false> R;
+    constexpr int NY = FUSE ? 2 : 0;
+    typedef RingCfg<CH, NY> R;
     constexpr int NW = x_warps(MODE);
-    typedef XSmem<J, CH, S, false, NW> SM;
+    typedef XSmem<J, CH, S, NY, NW> SM;
     constexpr int BOXW = Cfg::BOXW, BOXH = Cfg::BOXH, XOFF = Cfg::XOFF;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -562,6 +574,7 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
     __syncwarp();
     uint32_t box_phase = 0, ring_phase = 0;
     int stage = 0;
+    double nacc = 0.0;                                  // FUSE: this lane's share of ||v + s - y||^2
 
     // the NEXT item (index and descriptor) is fetched while the current one is processed
     unsigned item = x_next_item(p.counter, lane);
@@ -584,7 +597,7 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
             }
             int st = stage;
             for (int c = 0; c < S && c < nch; ++c) {
-                ring_issue<CH, false>(ring, rbar, st, p, nullptr, it.iter0, c, T);
+                ring_issue<CH, NY>(ring, rbar, st, p, p.s_in, p.yobs, nullptr, it.iter0, c, T);
                 st = st + 1 == S ? 0 : st + 1;
             }
         }
@@ -602,6 +615,7 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
         int left = T;                                   // iterations of the item not yet started
         int rem = 0;                                    // iterations left in the current chunk
         const float* rp = nullptr;                      // this lane's view of the current record
+        const float2* sp = nullptr;                     // FUSE: this lane's s of the current slot (y is CH*32 entries further)
         float2* yout = y + (size_t)it.iter0 * 32 + lane;
         for (int b = it.begin; b < it.end; ++b) {
             const uint2 h = hn;
@@ -612,6 +626,7 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
                 lwn = p.blane[(size_t)bn * 32 + lane];
             }
             const int n_iter = (int)(h.y & 0xFFFFu);
+            const int cnt = (int)(lw >> 16);
             const int ly = (lw >> 5) & 15, lx = lw & 31;
             const int cx = it.x0 + lx - p.Kh, cy = it.y0 + ly - p.Kh;       // cell = floor(u'), floor(v')
             const float2 cellf = make_float2((float)cx, (float)cy);
@@ -631,6 +646,7 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
                     rem = min(CH, left);
                     left -= rem;
                     rp = reinterpret_cast<const float*>(ring + stage * R::STAGE) + lane;
+                    if (FUSE) sp = reinterpret_cast<const float2*>(ring + stage * R::STAGE + R::REC) + lane;
                 }
                 const int seg = min(rem, n_iter - i);
                 int k = 0;
@@ -648,6 +664,16 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
 #pragma unroll
                     for (int v = 0; v < XVD; ++v) yout[v * 32] = o[v];
                     yout += XVD * 32;
+                    if (FUSE) {
+#pragma unroll
+                        for (int v = 0; v < XVD; ++v)
+                            if (i + k + v < cnt) {                          // a real slot: d = v + s - y
+                                const float2 sv = sp[v * 32], yv = sp[CH * 32 + v * 32];
+                                const float dx = (o[v].x + sv.x) - yv.x, dy = (o[v].y + sv.y) - yv.y;
+                                nacc += (double)(dx * dx + dy * dy);
+                            }
+                        sp += XVD * 32;
+                    }
                 }
                 for (; XVD > 1 && k < seg; ++k) {            // tail of the segment, one visibility at a time
                     const float2 uv1[1] = {*reinterpret_cast<const float2*>(rp + lane)};
@@ -657,19 +683,31 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
                     x_degrid_vis<J, DEG, MODE, 1>(uv1, w1, cellf, cx, cy, p, tab, B, o1);
                     *yout = o1[0];
                     yout += 32;
+                    if (FUSE) {
+                        if (i + k < cnt) {
+                            const float2 sv = sp[0], yv = sp[CH * 32];
+                            const float dx = (o1[0].x + sv.x) - yv.x, dy = (o1[0].y + sv.y) - yv.y;
+                            nacc += (double)(dx * dx + dy * dy);
+                        }
+                        sp += 32;
+                    }
                 }
                 i += seg;
                 rem -= seg;
                 if (rem == 0) {                                             // chunk consumed: refill its stage
                     __syncwarp();
                     if (cnext < nch) {
-                        if (lane == 0) ring_issue<CH, false>(ring, rbar, stage, p, nullptr, it.iter0, cnext, T);
+                        if (lane == 0) ring_issue<CH, NY>(ring, rbar, stage, p, p.s_in, p.yobs, nullptr, it.iter0, cnext, T);
                         ++cnext;
                     }
                     if (++stage == S) { stage = 0; ring_phase ^= 1; }
                 }
             }
         }
+    }
+    if (FUSE) {                                         // one fp64 atomic per warp
+        for (int o = 16; o > 0; o >>= 1) nacc += __shfl_down_sync(0xffffffffu, nacc, o);
+        if (lane == 0) atomicAdd(p.norm2, nacc);
     }
 }
 
@@ -682,14 +720,17 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
 // shared-memory atomics.  At the end of the item the box is added to the global grid with one
 // 8-byte reduction per non-zero cell (RED.ADD.F32x2; halos of neighbouring bands and the items of
 // one band meet there).
-template <int J, int DEG, int MODE, int CH, int S>
+// FUSE = 1 (f1): y is v = Phi x; s and the measurements are streamed too, the gridded vector z = v - r + s_new is formed
+// slot by slot (never stored) and s_new is written to p.s_out (kernels.cuh: admm_update_kernel has the formulas).
+template <int J, int DEG, int MODE, int CH, int S, int FUSE = 0>
 __global__ void __launch_bounds__(x_warps(MODE) * 32, MODE == 2 ? 1 : (J <= 6 ? 4 : 1))
 grid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, const float2* __restrict__ y) {
     typedef XCfg<J> Cfg;
-    typedef RingCfg<CH, true> R;
+    constexpr int NY = FUSE ? 3 : 1;
+    typedef RingCfg<CH, NY> R;
     constexpr int XVG = J == 4 ? XVG4 : XVG6;            // visibilities per trip
     constexpr int NW = x_warps(MODE);
-    typedef XSmem<J, CH, S, true, NW> SM;
+    typedef XSmem<J, CH, S, NY, NW> SM;
     constexpr int BOXW = Cfg::BOXW, BOXH = Cfg::BOXH, XOFF = Cfg::XOFF;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -711,6 +752,20 @@ grid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, const f
     __syncwarp();
     uint32_t ring_phase = 0;
     int stage = 0;
+    const float oma = FUSE ? (float)(1.0 - admm_alpha(*p.norm2, p.eps)) : 0.f, vrho = (float)p.varrho;
+    // one slot of the fused ADMM step: (v, s, y) -> z = v - r + s_new, s_new stored; padding slots give 0
+    auto admm_slot = [&](const float2* q, bool real_slot, float2* sdst) -> float2 {
+        float2 z = make_float2(0.f, 0.f), sn = z;
+        if (real_slot) {
+            const float2 vv = q[0], sv = q[CH * 32], yv = q[2 * CH * 32];
+            const float dx = (vv.x + sv.x) - yv.x, dy = (vv.y + sv.y) - yv.y;
+            const float vrx = oma * dx - sv.x, vry = oma * dy - sv.y;
+            sn = make_float2(sv.x + vrho * vrx, sv.y + vrho * vry);
+            z = make_float2(vrx + sn.x, vry + sn.y);
+        }
+        *sdst = sn;
+        return z;
+    };
 
     unsigned item = x_next_item(p.counter, lane);
     XItem nit = p.items[min(item, (unsigned)p.n_items - 1)];
@@ -724,7 +779,7 @@ grid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, const f
         if (lane == 0) {
             int st = stage;
             for (int c = 0; c < S && c < nch; ++c) {
-                ring_issue<CH, true>(ring, rbar, st, p, y, it.iter0, c, T);
+                ring_issue<CH, NY>(ring, rbar, st, p, y, p.s_in, p.yobs, it.iter0, c, T);
                 st = st + 1 == S ? 0 : st + 1;
             }
         }
@@ -733,6 +788,7 @@ grid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, const f
         __syncwarp();
         for (int i = lane; i < BOXW * BOXH; i += 32) tile[i] = make_float2(0.f, 0.f);
         __syncwarp();
+        float2* sout = FUSE ? p.s_out + (size_t)it.iter0 * 32 + lane : nullptr;
         int left = T, rem = 0;
         const float* rp = nullptr;
         const float2* yp = nullptr;
@@ -775,18 +831,29 @@ grid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, const f
                     for (int v = 0; v < XVG; ++v) {
                         uvk[v] = *reinterpret_cast<const float2*>(rp + v * REC_FLOATS + lane);
                         wk[v] = rp[v * REC_FLOATS + 64];
-                        yk[v] = yp[v * 32];
-                        if (live <= v) yk[v] = make_float2(0.f, 0.f);       // padding slot: whatever y holds there is ignored
+                        if (FUSE) {
+                            yk[v] = admm_slot(yp + v * 32, live > v, sout + v * 32);
+                        } else {
+                            yk[v] = yp[v * 32];
+                            if (live <= v) yk[v] = make_float2(0.f, 0.f);   // padding slot: whatever y holds there is ignored
+                        }
                     }
                     rp += XVG * REC_FLOATS;
                     yp += XVG * 32;
+                    if (FUSE) sout += XVG * 32;
                     x_grid_vis<J, DEG, MODE, XVG>(uvk, wk, yk, cellf, cx, cy, p, tab, A);
                 }
                 for (; XVG > 1 && k < seg; ++k, --live) {
                     const float2 uv1[1] = {*reinterpret_cast<const float2*>(rp + lane)};
                     const float w1[1] = {rp[64]};
-                    float2 y1[1] = {*yp};
-                    if (live <= 0) y1[0] = make_float2(0.f, 0.f);
+                    float2 y1[1];
+                    if (FUSE) {
+                        y1[0] = admm_slot(yp, live > 0, sout);
+                        sout += 32;
+                    } else {
+                        y1[0] = *yp;
+                        if (live <= 0) y1[0] = make_float2(0.f, 0.f);
+                    }
                     rp += REC_FLOATS;
                     yp += 32;
                     x_grid_vis<J, DEG, MODE, 1>(uv1, w1, y1, cellf, cx, cy, p, tab, A);
@@ -796,7 +863,7 @@ grid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, const f
                 if (rem == 0) {
                     __syncwarp();
                     if (cnext < nch) {
-                        if (lane == 0) ring_issue<CH, true>(ring, rbar, stage, p, y, it.iter0, cnext, T);
+                        if (lane == 0) ring_issue<CH, NY>(ring, rbar, stage, p, y, p.s_in, p.yobs, it.iter0, cnext, T);
                         ++cnext;
                     }
                     if (++stage == S) { stage = 0; ring_phase ^= 1; }

@@ -89,6 +89,7 @@ struct purify_op {
     void* x_ws = nullptr;     // n*n complex staging for host paths
     void* y_ws2 = nullptr;    // caller-order staging for host paths
     double* scal_ws = nullptr; // one fp64 scalar (norms)
+    bool admm_unfused = false; // opts.reserved[0] != 0: purify_admm_fidelity_step uses separate norm / update kernels
     cufftHandle plan = 0;
     bool plan_ok = false;
     CUtensorMap tmap;
@@ -208,6 +209,7 @@ pk::XParams make_xparams(const purify_op* op, bool caller_order) {
     p.table = (const float*)op->table;
     p.table_R = (float)op->table_R;
     p.table_len = op->table_len;
+    p.s_in = nullptr; p.yobs = nullptr; p.s_out = nullptr; p.norm2 = op->scal_ws; p.eps = 0.0; p.varrho = 0.0;
     return p;
 }
 
@@ -245,14 +247,17 @@ constexpr int X_CH_DEGRID = PURIFY_X_CHD, X_S_DEGRID = PURIFY_X_SD, X_CH_GRID = 
 constexpr int X_CH_DEGRID_T = 4, X_S_DEGRID_T = 2, X_CH_GRID_T = 3, X_S_GRID_T = 2;
 constexpr size_t X_TABLE_SMEM_MAX = 64 * 1024;
 
-template <int J, int DEG, int MODE, int CH, int S>
-int launch_degrid_x_m(purify_op* op, void* y, size_t extra_smem, cudaStream_t st) {
+struct AdmmArgs { const void* y_obs; void* s; double eps, varrho; };
+
+template <int J, int DEG, int MODE, int CH, int S, int FUSE = 0>
+int launch_degrid_x_m(purify_op* op, void* y, size_t extra_smem, cudaStream_t st, const AdmmArgs* aa = nullptr) {
     constexpr int NW = pk::x_warps(MODE);
-    const size_t smem = pk::XSmem<J, CH, S, false, NW>::TOTAL + extra_smem;
-    const pk::XParams p = make_xparams(op, false);
+    const size_t smem = pk::XSmem<J, CH, S, FUSE ? 2 : 0, NW>::TOTAL + extra_smem;
+    pk::XParams p = make_xparams(op, false);
+    if (aa) { p.s_in = (const float2*)aa->s; p.yobs = (const float2*)aa->y_obs; p.s_out = (float2*)aa->s; p.eps = aa->eps; p.varrho = aa->varrho; }
     CK(cudaMemsetAsync(op->x_counter, 0, sizeof(unsigned), st));
     int g = 0, rc;
-    auto kern = pk::degrid_x_kernel<J, DEG, MODE, CH, S>;
+    auto kern = pk::degrid_x_kernel<J, DEG, MODE, CH, S, FUSE>;
     if ((rc = x_grid_size(kern, NW * 32, smem, op->n_items, NW, &g))) return rc;
     kern<<<g, NW * 32, smem, st>>>(op->tmap_x, p, (float2*)y);
     op->launches++;
@@ -260,14 +265,15 @@ int launch_degrid_x_m(purify_op* op, void* y, size_t extra_smem, cudaStream_t st
     return PURIFY_OK;
 }
 
-template <int J, int DEG, int MODE, int CH, int S>
-int launch_grid_x_m(purify_op* op, const void* y, size_t extra_smem, cudaStream_t st) {
+template <int J, int DEG, int MODE, int CH, int S, int FUSE = 0>
+int launch_grid_x_m(purify_op* op, const void* y, size_t extra_smem, cudaStream_t st, const AdmmArgs* aa = nullptr) {
     constexpr int NW = pk::x_warps(MODE);
-    const size_t smem = pk::XSmem<J, CH, S, true, NW>::TOTAL + extra_smem;
-    const pk::XParams p = make_xparams(op, false);
+    const size_t smem = pk::XSmem<J, CH, S, FUSE ? 3 : 1, NW>::TOTAL + extra_smem;
+    pk::XParams p = make_xparams(op, false);
+    if (aa) { p.s_in = (const float2*)aa->s; p.yobs = (const float2*)aa->y_obs; p.s_out = (float2*)aa->s; p.eps = aa->eps; p.varrho = aa->varrho; }
     CK(cudaMemsetAsync(op->x_counter, 0, sizeof(unsigned), st));
     int g = 0, rc;
-    auto kern = pk::grid_x_kernel<J, DEG, MODE, CH, S>;
+    auto kern = pk::grid_x_kernel<J, DEG, MODE, CH, S, FUSE>;
     if ((rc = x_grid_size(kern, NW * 32, smem, op->n_items, NW, &g))) return rc;
     kern<<<g, NW * 32, smem, st>>>(op->tmap_x, p, (const float2*)y);
     op->launches++;
@@ -289,6 +295,33 @@ template <int J, int DEG> int launch_grid_x_t(purify_op* op, const void* y, cuda
     if (op->mode != PURIFY_KERNEL_TABLE) return launch_grid_x_m<J, DEG, 0, X_CH_GRID, X_S_GRID>(op, y, 0, st);
     if (tb <= X_TABLE_SMEM_MAX) return launch_grid_x_m<J, DEG, 2, X_CH_GRID_T, X_S_GRID_T>(op, y, tb, st);
     return launch_grid_x_m<J, DEG, 1, X_CH_GRID_T, X_S_GRID_T>(op, y, 0, st);
+}
+
+// f1, fused (complex64 batched layout, ANALYTIC weights): ring geometries that keep the occupancy of the plain kernels
+constexpr int X_CH_DEGRID_F = 6, X_S_DEGRID_F = 2, X_CH_GRID_F = 3, X_S_GRID_F = 2;
+
+int launch_degrid_fused(purify_op* op, void* v, const AdmmArgs& aa, cudaStream_t st) {
+    StageTimer t(op, PURIFY_STAGE_DEGRID, st);
+    if (op->n_items == 0) return PURIFY_OK;
+    switch (op->J) {
+        case 4: return launch_degrid_x_m<4, deg_c64(4), 0, X_CH_DEGRID_F, X_S_DEGRID_F, 1>(op, v, 0, st, &aa);
+        case 6: return launch_degrid_x_m<6, deg_c64(6), 0, X_CH_DEGRID_F, X_S_DEGRID_F, 1>(op, v, 0, st, &aa);
+        default: return launch_degrid_x_m<8, deg_c64(8), 0, X_CH_DEGRID_F, X_S_DEGRID_F, 1>(op, v, 0, st, &aa);
+    }
+}
+
+int launch_grid_fused(purify_op* op, const void* v, const AdmmArgs& aa, cudaStream_t st) {
+    {
+        StageTimer tz(op, PURIFY_STAGE_ZERO, st);
+        CK(cudaMemsetAsync(op->grid, 0, csize(op) * (size_t)op->K * op->K, st));
+    }
+    StageTimer t(op, PURIFY_STAGE_GRID, st);
+    if (op->n_items == 0) return PURIFY_OK;
+    switch (op->J) {
+        case 4: return launch_grid_x_m<4, deg_c64(4), 0, X_CH_GRID_F, X_S_GRID_F, 1>(op, v, 0, st, &aa);
+        case 6: return launch_grid_x_m<6, deg_c64(6), 0, X_CH_GRID_F, X_S_GRID_F, 1>(op, v, 0, st, &aa);
+        default: return launch_grid_x_m<8, deg_c64(8), 0, X_CH_GRID_F, X_S_GRID_F, 1>(op, v, 0, st, &aa);
+    }
 }
 
 int launch_degrid(purify_op* op, void* y, bool caller_order, cudaStream_t st) {
@@ -738,11 +771,13 @@ int create_impl(purify_op** out, int n, int oversample, int J, long long M, cons
     if (M > 0 && !uv) return fail(PURIFY_ERR_INVALID_ARG, "uv is NULL");
     if (dtype != PURIFY_C64 && dtype != PURIFY_C128) return fail(PURIFY_ERR_UNSUPPORTED, "unknown dtype %d", dtype);
     int mode = PURIFY_KERNEL_ANALYTIC, R = 4096, chunk = 4096, time_stages = 0;
+    bool admm_unfused = false;
     if (opts) {
         mode = opts->kernel_mode;
         if (opts->table_samples_per_unit) R = opts->table_samples_per_unit;
         if (opts->chunk) chunk = opts->chunk;
         time_stages = opts->time_stages;
+        admm_unfused = opts->reserved[0] != 0;
     }
     if (mode != PURIFY_KERNEL_ANALYTIC && mode != PURIFY_KERNEL_TABLE)
         return fail(PURIFY_ERR_UNSUPPORTED, "unknown kernel mode %d", mode);
@@ -754,7 +789,7 @@ int create_impl(purify_op** out, int n, int oversample, int J, long long M, cons
     purify_op* op = new (std::nothrow) purify_op();
     if (!op) return fail(PURIFY_ERR_ALLOC, "host allocation failed");
     op->n = n; op->K = 2 * n; op->J = J; op->M = M; op->dtype = dtype; op->mode = mode; op->table_R = R;
-    op->chunk = chunk; op->time_stages = time_stages;
+    op->chunk = chunk; op->time_stages = time_stages; op->admm_unfused = admm_unfused;
     cudaStream_t st = (cudaStream_t)stream;
 
     void *uv_tmp = nullptr, *w_tmp = nullptr;
@@ -1056,6 +1091,27 @@ int purify_admm_fidelity_step(purify_op* op, const void* x_dev, const void* y_na
     RUN(ensure_ws(op, &op->y_ws, csize(op) * (size_t)Mn));
     RUN(ensure_ws(op, &op->y_ws2, csize(op) * (size_t)(Mn > op->M ? Mn : op->M)));
     RUN(ensure_ws(op, (void**)&op->scal_ws, sizeof(double)));
+    if (op->batched && op->mode == PURIFY_KERNEL_ANALYTIC && !op->admm_unfused) {
+        // fused form: the norm is accumulated inside the degridding kernel, r / s_new / z are formed slot by slot inside
+        // the gridding kernel (z is never stored); two passes over the M-sized vectors less than the unfused form below
+        if (((uintptr_t)y_native_dev & 15u) || ((uintptr_t)s_native_dev & 15u))
+            return fail(PURIFY_ERR_INVALID_ARG, "y_native and s_native must be 16-byte aligned for the complex64 layout");
+        const AdmmArgs aa = {y_native_dev, s_native_dev, epsilon, varrho};
+        CK(cudaMemsetAsync(op->scal_ws, 0, sizeof(double), st));
+        RUN(launch_pad(op, x_dev, st));
+        RUN(launch_fft(op, CUFFT_FORWARD, st));
+        RUN(launch_degrid_fused(op, op->y_ws, aa, st));
+        RUN(launch_grid_fused(op, op->y_ws, aa, st));
+        RUN(launch_fft(op, CUFFT_INVERSE, st));
+        RUN(launch_crop(op, g_dev, st));
+        if (resid_norm_out) {
+            double n2 = 0.0;
+            CK(cudaMemcpyAsync(&n2, op->scal_ws, sizeof(double), cudaMemcpyDeviceToHost, st));
+            CK(cudaStreamSynchronize(st));
+            *resid_norm_out = sqrt(n2);
+        }
+        return PURIFY_OK;
+    }
     const unsigned* pm = op->batched ? op->perm : nullptr;     // padding mask (complex64 layout only)
     // line 3: v = Phi x
     RUN(degrid_impl(op, x_dev, op->y_ws, false, st));

@@ -317,15 +317,15 @@ def test_operator_norm_power_method(dtype):
     op.close()
 
 
-@pytest.mark.parametrize("dtype", ["c128", "c64"])
+@pytest.mark.parametrize("dtype,unfused", [("c128", False), ("c64", False), ("c64", True)])
 @pytest.mark.parametrize("case", ["outside", "inside", "eps0"])
-def test_admm_fidelity_step(dtype, case):
+def test_admm_fidelity_step(dtype, unfused, case):
     """f1 (Algorithm 1 lines 3-6): purify_admm_fidelity_step against the oracle - g, the updated dual
     variable and the residual norm; native-order vectors, garbage in the padding entries of y and s."""
     cfg, x, uv, w = synth.make_problem(2, M=30000, J=6)
     x, uv, w = cast_problem(x, uv, w, dtype)
     M = len(uv)
-    op = make_op(cfg.n, 6, uv, w, dtype)
+    op = make_op(cfg.n, 6, uv, w, dtype, admm_unfused=unfused)     # c64 default: the fused kernels
     y = synth.random_complex((M,), seed=51, dtype=dtype)
     s = (synth.random_complex((M,), seed=52, dtype=dtype) * 0.25).astype(y.dtype)
     v = oracle.degrid(x, uv, w, 6, idx_prec=idx_prec(dtype))
