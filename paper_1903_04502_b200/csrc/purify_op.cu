@@ -1068,7 +1068,10 @@ int purify_op_norm(purify_op* op, const void* x0_dev, int max_iter, double rel_t
         RUN(normalise());                               // ||x|| = 1
         RUN(degrid_impl(op, op->x_ws, op->y_ws, false, st));
         RUN(grid_impl(op, op->y_ws, op->x_ws, false, st));       // x <- Phi^dagger Phi x
-        RUN(norm2(op->x_ws, &n2));
+        // the host only needs lambda_k for the stopping rule (or after the last iteration): no sync otherwise
+        const bool need = rel_tol > 0.0 || it == max_iter;
+        RUN(norm2(op->x_ws, need ? &n2 : nullptr));
+        if (!need) continue;
         prev = lambda;
         lambda = sqrt(n2);                              // ||Phi^dagger Phi x|| with ||x|| = 1 -> largest eigenvalue
         if (!(lambda > 0.0) || (it > 1 && fabs(lambda - prev) <= rel_tol * lambda)) break;
