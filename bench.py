@@ -312,7 +312,7 @@ def run_ours(args):
     lam, its = op.norm(None, max_iter=10, rel_tol=0.0)
     torch.cuda.synchronize()
     norm_info = {"lambda_after_10_iterations": lam, "ms_per_iteration": (time.perf_counter() - t0) * 1e3 / max(its, 1),
-                 "note": "purify_op_norm: Phi^dagger Phi + fp64 norm + scaling per iteration, host-synchronised every iteration"}
+                 "note": "purify_op_norm: Phi^dagger Phi + fp64 norm + scaling per iteration (wall clock of the call / iterations)"}
 
     # ---- f1: Algorithm 1 lines 3-6 around the operator (fused for complex64 + analytic weights), native-order vectors
     y_obs = op.degrid(x_dev, native=True)

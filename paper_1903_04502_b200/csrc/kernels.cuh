@@ -326,6 +326,12 @@ __global__ void __launch_bounds__(256) norm2_kernel(const typename Cplx<R>::type
     }
 }
 
+template <typename R>
+__global__ void __launch_bounds__(256) fill_ones_kernel(typename Cplx<R>::type* __restrict__ x, long long count) {
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < count; i += (long long)gridDim.x * blockDim.x)
+        x[i] = mk2<R>((R)1, (R)0);
+}
+
 // y = x / sqrt(*norm2) (y may alias x); a zero vector is left unchanged
 template <typename R>
 __global__ void __launch_bounds__(256) normalise_kernel(const typename Cplx<R>::type* __restrict__ x,

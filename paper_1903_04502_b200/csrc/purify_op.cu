@@ -1054,11 +1054,10 @@ int purify_op_norm(purify_op* op, const void* x0_dev, int max_iter, double rel_t
     if (x0_dev) {
         CK(cudaMemcpyAsync(op->x_ws, x0_dev, xb, cudaMemcpyDeviceToDevice, st));
     } else {
-        std::vector<unsigned char> ones(xb);
-        if (f32) { float2* p = (float2*)ones.data(); for (long long i = 0; i < N; ++i) p[i] = make_float2(1.f, 0.f); }
-        else { double2* p = (double2*)ones.data(); for (long long i = 0; i < N; ++i) p[i] = make_double2(1.0, 0.0); }
-        CK(cudaMemcpyAsync(op->x_ws, ones.data(), xb, cudaMemcpyHostToDevice, st));
-        CK(cudaStreamSynchronize(st));
+        if (f32) pk::fill_ones_kernel<float><<<grid_for(N, 256, 148 * 8), 256, 0, st>>>((float2*)op->x_ws, N);
+        else pk::fill_ones_kernel<double><<<grid_for(N, 256, 148 * 8), 256, 0, st>>>((double2*)op->x_ws, N);
+        op->launches++;
+        CK(cudaGetLastError());
     }
     double lambda = 0.0, prev = 0.0, n2 = 0.0;
     int it = 0;
