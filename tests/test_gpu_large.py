@@ -102,3 +102,27 @@ def test_config5_full_size_table_mode():
     kernel table with 4096 samples per unit."""
     cfg, x, uv, w = synth.make_problem(5)
     full_size_checks(cfg, x, uv, w, "c64")
+
+
+def test_config4_admm_fidelity_step_full_size():
+    """f1 at the metric's config (fused complex64 kernels, the launch configuration bench.py times): g, the updated dual
+    variable and the residual norm against the oracle over all 1e8 visibilities."""
+    from paper_1903_04502_b200 import C64, PurifyOp
+    cfg, x, uv, w = synth.make_problem(4)
+    M = cfg.M
+    op = PurifyOp(cfg.n, cfg.J, torch.from_numpy(uv).cuda(), torch.from_numpy(w).cuda(), dtype=C64)
+    y = synth.random_complex((M,), seed=61, dtype="c64")
+    s = (synth.random_complex((M,), seed=62, dtype="c64") * np.float32(0.2)).astype(np.complex64)
+    v = oracle.degrid(x, uv, w, cfg.J, idx_prec=32)
+    eps = 0.5 * float(np.sqrt(sum(float(np.vdot(d, d).real) for d in
+                                  ((v[i:i + (1 << 24)] + s[i:i + (1 << 24)] - y[i:i + (1 << 24)]) for i in range(0, M, 1 << 24)))))
+    del v
+    g_ref, s_ref, _, nrm_ref = oracle.admm_fidelity_step(x, y, s, uv, w, cfg.n, cfg.J, eps, 0.9, idx_prec=32)
+    y_nat = op.permute_to_native(torch.from_numpy(y).cuda())
+    s_nat = op.permute_to_native(torch.from_numpy(s).cuda())
+    g, nrm = op.admm_fidelity_step(torch.from_numpy(x).cuda(), y_nat, s_nat, eps, 0.9)
+    assert abs(nrm - nrm_ref) <= 1e-5 * nrm_ref
+    assert rel_l2(g.cpu().numpy(), g_ref) <= 4e-5
+    s_out = op.permute_from_native(s_nat).cpu().numpy()
+    assert rel_l2(s_out, s_ref) <= 4e-5
+    op.close()
