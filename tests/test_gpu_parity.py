@@ -185,9 +185,10 @@ def test_integer_and_half_integer_uv_tie_break():
         run_all_checks(x, uv, None, 6, dtype, mode="table", R=4096)
 
 
-@pytest.mark.parametrize("n", [48, 50, 22])
+@pytest.mark.parametrize("n", [48, 50, 22, 8, 6])
 def test_non_power_of_two_grid(n):
-    """K = 96 (multiple of the tile), K = 100 and K = 44 (ragged edge tiles, non-power-of-two wrap)."""
+    """K = 96 (multiple of the tile), K = 100 and K = 44 (ragged edge tiles, non-power-of-two wrap), K = 16 and K = 12
+    (grid smaller than one band box: every box wraps, some of them more than once)."""
     K = 2 * n
     x = synth.random_complex((n, n), seed=n)
     rng = synth.rng_for(n, 2)
