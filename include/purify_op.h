@@ -63,7 +63,8 @@ typedef struct {
     int table_samples_per_unit; /* TABLE mode: samples per grid cell R; default 4096
                                    (BASELINE.json configs[4]); paper used 2e5.
                                    T[i] = g(i/R), i = 0..R*J/2+1, lookup T[floor(|d| R + 1/2)].      */
-    int chunk;                  /* visibilities per work item (CTA); default 4096                    */
+    int chunk;                  /* complex128 (tile-sorted layout): visibilities per work item (CTA); default 4096.
+                                   Ignored by the complex64 layout (items of 64 iterations x 32 lanes)      */
     int time_stages;            /* != 0: record CUDA events around each stage                        */
     int reserved[4];            /* reserved[0] != 0: purify_admm_fidelity_step runs its unfused form (separate norm and
                                    update kernels) even where the fused kernels exist; others must be 0              */

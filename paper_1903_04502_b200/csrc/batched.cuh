@@ -26,6 +26,11 @@
 //          ITERATION: 32 x (u, v) then 32 x w = 384 bytes, so a chunk of iterations is ONE bulk copy.
 //   item   a run of batches of one band with about ITEM_ITERS (64) iterations: the unit of dynamic
 //          scheduling (persistent warps pull items from an atomic counter); its slots are contiguous.
+//
+// Kernels: degrid_x_kernel (a3) and grid_x_kernel (a4), templated on the taps J, the polynomial
+// degree, the weight MODE (0 analytic polynomial, 1 table in global memory, 2 table in shared memory), the ring
+// geometry (CH iterations per chunk, S stages) and FUSE (1: the ADMM data-fidelity step of Algorithm 1 lines 3-6 is
+// folded in - residual norm in a3; projection, dual update and residual in a4).
 #pragma once
 #include "kernels.cuh"
 
