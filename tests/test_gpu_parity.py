@@ -347,3 +347,48 @@ def test_admm_fidelity_step(dtype, unfused, case):
     assert rel_l2(s_out[valid], s_ref[perm[valid]]) <= 4 * tol
     assert not np.any(s_out[~valid])
     op.close()
+
+
+@pytest.mark.parametrize("seed", list(range(10)))
+def test_fuzz_batched_layout(seed):
+    """Random small problems for the complex64 batched layout: random grid side, taps, M, and a (u, v) mixture of a
+    uniform background, a few very hot cells (many full units -> layers, flagged batches, several items per band),
+    exact integers / half-integers and far-out-of-period points.  Phi, Phi^dagger (native order) and the ADMM step
+    against the oracle."""
+    rng = synth.rng_for(9000 + seed, synth.STREAM_UV)
+    n = int(rng.choice([16, 24, 34, 50, 64, 80]))
+    J = int(rng.choice([4, 6, 8]))
+    K = 2 * n
+    parts = [rng.uniform(-K / 2, K / 2, size=(int(rng.integers(1, 6000)), 2))]
+    for _ in range(int(rng.integers(0, 5))):
+        c = rng.integers(-K // 2, K // 2, size=2).astype(np.float64)
+        parts.append(c + rng.uniform(0, 1, size=(int(rng.integers(1, 3000)), 2)))
+    parts.append(rng.integers(-K, K, size=(int(rng.integers(0, 40)), 2)).astype(np.float64) * 0.5)
+    parts.append(rng.uniform(-5 * K, 5 * K, size=(int(rng.integers(0, 40)), 2)))
+    uv = np.concatenate(parts)
+    uv = uv[rng.permutation(len(uv))].astype(np.float32)
+    w = rng.uniform(0.5, 1.5, size=len(uv)).astype(np.float32)
+    x = synth.random_complex((n, n), seed=seed, dtype="c64")
+    M = len(uv)
+    op = make_op(n, J, uv, w, "c64")
+    perm = host(op.permutation())
+    valid = perm >= 0
+    assert sorted(perm[valid].tolist()) == list(range(M))
+    y_ref = oracle.degrid(x, uv, w, J, idx_prec=32)
+    y_nat = host(op.degrid(dev(x), native=True))
+    assert rel_l2(y_nat[valid], y_ref[perm[valid]]) <= 1e-5
+    yv = synth.random_complex((M,), seed=100 + seed, dtype="c64")
+    img_ref = oracle.grid(yv, uv, w, n, J, idx_prec=32)
+    yv_nat = np.zeros(len(perm), dtype=np.complex64)
+    yv_nat[valid] = yv[perm[valid]]
+    assert rel_l2(host(op.grid(dev(yv_nat), native=True)), img_ref) <= 1e-5
+    s = (synth.random_complex((M,), seed=200 + seed, dtype="c64") * np.float32(0.3)).astype(np.complex64)
+    eps = 0.5 * float(np.linalg.norm(y_ref + s - yv))
+    g_ref, s_ref, _, nrm_ref = oracle.admm_fidelity_step(x, yv, s, uv, w, n, J, eps, 0.7, idx_prec=32)
+    s_nat = np.zeros(len(perm), dtype=np.complex64)
+    s_nat[valid] = s[perm[valid]]
+    s_dev = dev(s_nat)
+    g, nrm = op.admm_fidelity_step(dev(x), dev(yv_nat), s_dev, eps, 0.7)
+    assert abs(nrm - nrm_ref) <= 1e-4 * nrm_ref
+    assert rel_l2(host(g), g_ref) <= 4e-5 and rel_l2(host(s_dev)[valid], s_ref[perm[valid]]) <= 4e-5
+    op.close()
