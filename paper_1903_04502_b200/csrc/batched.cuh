@@ -490,6 +490,18 @@ __device__ __forceinline__ unsigned x_next_item(unsigned* counter, int lane) {
     return __shfl_sync(0xffffffffu, it, 0);
 }
 
+// a0.6: longest items first (LPT order of the dynamic queue: the tail of a launch then consists of short items).
+__global__ void item_key_kernel(const XItem* __restrict__ items, int n_items, unsigned* __restrict__ key, unsigned* __restrict__ idx) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_items) return;
+    key[i] = 0xFFFFu - min(items[i].iters, 0xFFFFu);
+    idx[i] = (unsigned)i;
+}
+__global__ void item_gather_kernel(const XItem* __restrict__ in, const unsigned* __restrict__ idx, int n_items, XItem* __restrict__ out) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n_items) out[i] = in[idx[i]];
+}
+
 // ---------------------------------------------------------------------------------------------
 // Visibility stream ring.  The slots of one item are contiguous in HBM, so every warp streams them
 // through a private ring of S stages in shared memory, each filled by 1-D bulk copies

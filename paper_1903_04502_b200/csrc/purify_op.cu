@@ -664,6 +664,36 @@ int build_bins_x(purify_op* op, const void* uv_dev, const void* w_dev, cudaStrea
         CKC(cudaGetLastError());
         pk::item_iters_kernel<<<(op->n_items + 255) / 256, 256, 0, st>>>(op->x_items, op->n_items, op->x_bhdr);
         CKC(cudaGetLastError());
+        // Few items per persistent warp (< 16): longest items first, so that the tail of a launch consists of short items
+        // (config 3: -9 %).  With many items per warp the band order is kept: it is friendlier to L2 / DRAM pages
+        // (config 4 and 5 lose 1-3 % when reordered).  Stable sort: band order inside one length class.
+        if (op->n_items < 16 * 148 * 16) {
+            const int ni = op->n_items;
+            unsigned *ik = nullptr, *ik2 = nullptr, *ii = nullptr, *ii2 = nullptr;
+            pk::XItem* sorted = nullptr;
+            void* tmp = nullptr;
+            size_t tb = 0;
+            auto free5 = [&]() { cudaFree(ik); cudaFree(ik2); cudaFree(ii); cudaFree(ii2); cudaFree(tmp); };
+            cudaError_t e = cudaMalloc(&ik, sizeof(unsigned) * ni);
+            if (e == cudaSuccess) e = cudaMalloc(&ik2, sizeof(unsigned) * ni);
+            if (e == cudaSuccess) e = cudaMalloc(&ii, sizeof(unsigned) * ni);
+            if (e == cudaSuccess) e = cudaMalloc(&ii2, sizeof(unsigned) * ni);
+            if (e == cudaSuccess) e = cudaMalloc((void**)&sorted, sizeof(pk::XItem) * ni);
+            if (e == cudaSuccess) e = cub::DeviceRadixSort::SortPairs(nullptr, tb, ik, ik2, ii, ii2, ni, 0, 16, st);
+            if (e == cudaSuccess) e = cudaMalloc(&tmp, tb ? tb : 16);
+            if (e == cudaSuccess) {
+                pk::item_key_kernel<<<(ni + 255) / 256, 256, 0, st>>>(op->x_items, ni, ik, ii);
+                e = cub::DeviceRadixSort::SortPairs(tmp, tb, ik, ik2, ii, ii2, ni, 0, 16, st);
+            }
+            if (e == cudaSuccess) {
+                pk::item_gather_kernel<<<(ni + 255) / 256, 256, 0, st>>>(op->x_items, ii2, ni, sorted);
+                e = cudaStreamSynchronize(st);
+            }
+            if (e == cudaSuccess) { cudaFree(op->x_items); op->x_items = sorted; sorted = nullptr; }
+            cudaFree(sorted);
+            free5();
+            CKC(e);
+        }
         pk::slot_fill_kernel<<<grid_for((long long)op->n_batches * 32, 256), 256, 0, st>>>(
             op->x_bhdr, op->x_blane, lsrc, op->n_batches, perm0, (const float2*)uv_dev, (const float*)w_dev, K,
             op->perm, (float*)op->uv_s);
