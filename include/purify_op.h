@@ -67,7 +67,9 @@ typedef struct {
                                    Ignored by the complex64 layout (items of 64 iterations x 32 lanes)      */
     int time_stages;            /* != 0: record CUDA events around each stage                        */
     int reserved[4];            /* reserved[0] != 0: purify_admm_fidelity_step runs its unfused form (separate norm and
-                                   update kernels) even where the fused kernels exist; others must be 0              */
+                                   update kernels) even where the fused kernels exist; reserved[1] != 0: complex128 uses
+                                   the tile-sorted kernels for every J (default: batched layout for J <= 6, tile-sorted
+                                   for J = 8); others must be 0                                                      */
 } purify_opts;
 
 /* Facts about a handle (for tests, benches and roofline arithmetic). */

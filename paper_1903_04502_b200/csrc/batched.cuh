@@ -74,38 +74,41 @@ struct XItem {
     int pad0, pad1;
 };
 
-struct XParams {
-    float2* grid;                 // K*K, internal layout
+template <typename F> struct XParamsT {
+    typedef typename Cplx<F>::type F2;
+    F2* grid;                 // K*K, internal layout
     int K, Kh, kmask;
     const XItem* items;
     int n_items;
     unsigned* counter;            // dynamic item queue (reset before every launch)
     const uint2* bhdr;            // per batch: x = first iteration, y = n_iter | flags << 16 (bit 0: a cell may occur twice)
     const unsigned* blane;        // per batch 32 lane words: cell (ly << 5 | lx) | count << 16
-    const float* rec;             // per-iteration records (REC_FLOATS floats each)
-    KbCoef<float> coef;
-    const float* table;
-    float table_R;
+    const F* rec;             // per-iteration records (REC_FLOATS floats each)
+    KbCoef<F> coef;
+    const F* table;
+    F table_R;
     int table_len;
     // f1 (fused ADMM data-fidelity step): dual variable s (in / out), measurements y, ||v + s - y||^2, radius, step
-    const float2* s_in;
-    const float2* yobs;
-    float2* s_out;
+    const F2* s_in;
+    const F2* yobs;
+    F2* s_out;
     double* norm2;
     double eps, varrho;
 };
+typedef XParamsT<float> XParams;
 
 // ---------------------------------------------------------------------------------------------
 // a0.1: reduce (u, v) to the principal period, key = band * 512 + cell (band-major).
-__global__ void xkey_kernel(const float2* __restrict__ uv, long long M, int K, int nbx,
+template <typename F>
+__global__ void xkey_kernel(const typename Cplx<F>::type* __restrict__ uv, long long M, int K, int nbx,
                             unsigned* __restrict__ keys, unsigned* __restrict__ idx, int* __restrict__ bad) {
     for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < M; k += (long long)gridDim.x * blockDim.x) {
-        const float2 c = uv[k];
+        const typename Cplx<F>::type c = uv[k];
         unsigned key = 0;
-        if (!(fabsf(c.x) < 1073741824.0f) || !(fabsf(c.y) < 1073741824.0f)) {
+        if (!(fabs(c.x) < (F)1073741824.0) || !(fabs(c.y) < (F)1073741824.0)) {
             atomicOr(bad, 1);
         } else {
-            const long long fx = (long long)floorf(c.x) + K / 2, fy = (long long)floorf(c.y) + K / 2;
+            const long long fx = (long long)floor_r(c.x) + K / 2, fy = (long long)floor_r(c.y) + K / 2;
             long long gx = fx % K, gy = fy % K;
             if (gx < 0) gx += K;
             if (gy < 0) gy += K;
@@ -118,12 +121,12 @@ __global__ void xkey_kernel(const float2* __restrict__ uv, long long M, int K, i
 }
 
 // principal-period coordinate: u - m K with m = floor((floor(u) + K/2) / K); exact (double arithmetic,
-// the result is a multiple of ulp(u) of small magnitude, hence a float).
-__device__ __forceinline__ float x_reduce(float u, int K) {
-    const long long f = (long long)floorf(u) + K / 2;
+// the result is a multiple of ulp(u) of small magnitude, hence representable).
+template <typename F> __device__ __forceinline__ F x_reduce(F u, int K) {
+    const long long f = (long long)floor_r(u) + K / 2;
     long long m = f / K;
     if (f % K < 0) --m;
-    return (float)((double)u - (double)m * (double)K);
+    return (F)((double)u - (double)m * (double)K);
 }
 
 __global__ void band_start_kernel(const unsigned* __restrict__ keys, long long M, int n_bands, unsigned* __restrict__ band_start) {
@@ -311,10 +314,11 @@ __global__ void split_totals_kernel(const BandTotals* __restrict__ t, int n_band
 
 // a0.4: fill the slots of every batch (one warp per batch): permutation and the per-iteration
 // records (reduced (u, v), weights).
+template <typename F>
 __global__ void __launch_bounds__(256)
 slot_fill_kernel(const uint2* __restrict__ bhdr, const unsigned* __restrict__ blane, const unsigned* __restrict__ lsrc,
-                 unsigned n_batches, const unsigned* __restrict__ perm0, const float2* __restrict__ uv,
-                 const float* __restrict__ w, int K, unsigned* __restrict__ perm, float* __restrict__ rec) {
+                 unsigned n_batches, const unsigned* __restrict__ perm0, const typename Cplx<F>::type* __restrict__ uv,
+                 const F* __restrict__ w, int K, unsigned* __restrict__ perm, F* __restrict__ rec) {
     const unsigned warps = (gridDim.x * blockDim.x) >> 5;
     const int lane = threadIdx.x & 31;
     for (unsigned b = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; b < n_batches; b += warps) {
@@ -322,25 +326,25 @@ slot_fill_kernel(const uint2* __restrict__ bhdr, const unsigned* __restrict__ bl
         const unsigned n_iter = h.y & 0xFFFFu;
         const unsigned lw = blane[(size_t)b * 32 + lane], src = lsrc[(size_t)b * 32 + lane];
         const unsigned cnt = lw >> 16;
-        float2 pad = make_float2(0.f, 0.f);
+        typename Cplx<F>::type pad = mk2<F>((F)0, (F)0);
         if (cnt > 0) {                                     // padding coordinate: the unit's first visibility
-            const float2 c = uv[perm0[src]];
-            pad = make_float2(x_reduce(c.x, K), x_reduce(c.y, K));
+            const typename Cplx<F>::type c = uv[perm0[src]];
+            pad = mk2<F>(x_reduce<F>(c.x, K), x_reduce<F>(c.y, K));
         }
         for (unsigned i = 0; i < n_iter; ++i) {
             const size_t it = (size_t)h.x + i;
-            float* r = rec + it * REC_FLOATS;
-            float2 c = pad;
-            float wv = 0.f;
+            F* r = rec + it * REC_FLOATS;
+            typename Cplx<F>::type c = pad;
+            F wv = (F)0;
             unsigned pi = PERM_PAD;
             if (i < cnt) {
                 pi = perm0[src + i];
-                const float2 c0 = uv[pi];
-                c = make_float2(x_reduce(c0.x, K), x_reduce(c0.y, K));
-                wv = w ? w[pi] : 1.f;
+                const typename Cplx<F>::type c0 = uv[pi];
+                c = mk2<F>(x_reduce<F>(c0.x, K), x_reduce<F>(c0.y, K));
+                wv = w ? w[pi] : (F)1;
             }
             perm[it * 32 + lane] = pi;
-            reinterpret_cast<float2*>(r)[lane] = c;
+            reinterpret_cast<typename Cplx<F>::type*>(r)[lane] = c;
             r[64 + lane] = wv;
         }
     }
@@ -354,26 +358,33 @@ __global__ void item_iters_kernel(XItem* __restrict__ items, int n_items, const 
     items[i].iters = h.x + (h.y & 0xFFFFu) - items[i].iter0;
 }
 
+template <typename F> using C2 = typename Cplx<F>::type;
+
 // ---------------------------------------------------------------------------------------------
 // packed fp32 helpers (sm_100 FFMA2 / FMUL2 / FADD2)
 __device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
 __device__ __forceinline__ float2 mul2(float2 a, float2 b) { return __fmul2_rn(a, b); }
 __device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
 __device__ __forceinline__ float2 dup2(float a) { return make_float2(a, a); }
+// the same vocabulary for complex128 (component-wise fp64; no packed instructions exist)
+__device__ __forceinline__ double2 fma2(double2 a, double2 b, double2 c) { return make_double2(fma(a.x, b.x, c.x), fma(a.y, b.y, c.y)); }
+__device__ __forceinline__ double2 mul2(double2 a, double2 b) { return make_double2(a.x * b.x, a.y * b.y); }
+__device__ __forceinline__ double2 add2(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ double2 dup2(double a) { return make_double2(a, a); }
 
 // Kernel weights of both axes of one visibility in a known cell: g[j] = (g_x[j], g_y[j]) for the taps
 // c_j = cell - J/2 + 1 + j.  ANALYTIC: t = (u - cell) - 1/2 per axis, the even / odd Horner chains of
 // the two axes run as one packed chain.  TABLE: T[floor(|u - c_j| R + 1/2)], one IEEE op per step.
-template <int J, int DEG, int MODE>
-__device__ __forceinline__ void x_weights(float2 uv, float2 cellf, int cx, int cy, const XParams& p, const float* tab,
-                                          float2 (&g)[J]) {
+template <typename F, int J, int DEG, int MODE>
+__device__ __forceinline__ void x_weights(C2<F> uv, C2<F> cellf, int cx, int cy, const XParamsT<F>& p, const F* tab,
+                                          C2<F> (&g)[J]) {
     if (MODE == 0) {
         constexpr int NE = DEG / 2 + 1, NO = (DEG + 1) / 2;
-        const float2 t = add2(add2(uv, make_float2(-cellf.x, -cellf.y)), make_float2(-0.5f, -0.5f));
-        const float2 t2 = mul2(t, t), nt = make_float2(-t.x, -t.y);
+        const C2<F> t = add2(add2(uv, mk2<F>(-cellf.x, -cellf.y)), mk2<F>((F)-0.5, (F)-0.5));
+        const C2<F> t2 = mul2(t, t), nt = mk2<F>(-t.x, -t.y);
 #pragma unroll
         for (int j = 0; j < J / 2; ++j) {
-            float2 E = dup2(p.coef.e[j][NE - 1]), O = dup2(p.coef.o[j][NO - 1]);
+            C2<F> E = dup2(p.coef.e[j][NE - 1]), O = dup2(p.coef.o[j][NO - 1]);
 #pragma unroll
             for (int m = NE - 2; m >= 0; --m) E = fma2(E, t2, dup2(p.coef.e[j][m]));
 #pragma unroll
@@ -385,33 +396,33 @@ __device__ __forceinline__ void x_weights(float2 uv, float2 cellf, int cx, int c
 #pragma unroll
         for (int j = 0; j < J; ++j) {
             const int ox = cx - J / 2 + 1 + j, oy = cy - J / 2 + 1 + j;
-            const float dx = __fsub_rn(uv.x, (float)ox), dy = __fsub_rn(uv.y, (float)oy);
-            const int ix = (int)floorf(__fadd_rn(__fmul_rn(fabsf(dx), p.table_R), 0.5f));
-            const int iy = (int)floorf(__fadd_rn(__fmul_rn(fabsf(dy), p.table_R), 0.5f));
+            const F dx = sub_rn(uv.x, (F)ox), dy = sub_rn(uv.y, (F)oy);
+            const int ix = (int)floor_r(add_rn(mul_rn(fabs(dx), p.table_R), (F)0.5));
+            const int iy = (int)floor_r(add_rn(mul_rn(fabs(dy), p.table_R), (F)0.5));
             // MODE 1: table in global memory (read through L1); MODE 2: the CTA's copy in shared memory
-            g[j].x = ix < p.table_len ? (MODE == 2 ? tab[ix] : __ldg(tab + ix)) : 0.f;
-            g[j].y = iy < p.table_len ? (MODE == 2 ? tab[iy] : __ldg(tab + iy)) : 0.f;
+            g[j].x = ix < p.table_len ? (MODE == 2 ? tab[ix] : __ldg(tab + ix)) : (F)0;
+            g[j].y = iy < p.table_len ? (MODE == 2 ? tab[iy] : __ldg(tab + iy)) : (F)0;
         }
     }
 }
 
 // Kernel weights of V visibilities of one cell, written statement-interleaved so that the V dependency
 // graphs advance together (ANALYTIC; TABLE evaluates visibility by visibility).
-template <int J, int DEG, int MODE, int V>
-__device__ __forceinline__ void x_weights_v(const float2 (&uv)[V], float2 cellf, int cx, int cy, const XParams& p,
-                                            const float* tab, float2 (&g)[V][J]) {
+template <typename F, int J, int DEG, int MODE, int V>
+__device__ __forceinline__ void x_weights_v(const C2<F> (&uv)[V], C2<F> cellf, int cx, int cy, const XParamsT<F>& p,
+                                            const F* tab, C2<F> (&g)[V][J]) {
     if (MODE == 0) {
         constexpr int NE = DEG / 2 + 1, NO = (DEG + 1) / 2;
-        float2 t[V], t2[V], nt[V];
+        C2<F> t[V], t2[V], nt[V];
 #pragma unroll
         for (int v = 0; v < V; ++v) {
-            t[v] = add2(add2(uv[v], make_float2(-cellf.x, -cellf.y)), make_float2(-0.5f, -0.5f));
+            t[v] = add2(add2(uv[v], mk2<F>(-cellf.x, -cellf.y)), mk2<F>((F)-0.5, (F)-0.5));
             t2[v] = mul2(t[v], t[v]);
-            nt[v] = make_float2(-t[v].x, -t[v].y);
+            nt[v] = mk2<F>(-t[v].x, -t[v].y);
         }
 #pragma unroll
         for (int j = 0; j < J / 2; ++j) {
-            float2 E[V], O[V];
+            C2<F> E[V], O[V];
 #pragma unroll
             for (int v = 0; v < V; ++v) { E[v] = dup2(p.coef.e[j][NE - 1]); O[v] = dup2(p.coef.o[j][NO - 1]); }
 #pragma unroll
@@ -427,18 +438,18 @@ __device__ __forceinline__ void x_weights_v(const float2 (&uv)[V], float2 cellf,
         }
     } else {
 #pragma unroll
-        for (int v = 0; v < V; ++v) x_weights<J, DEG, MODE>(uv[v], cellf, cx, cy, p, tab, g[v]);
+        for (int v = 0; v < V; ++v) x_weights<F, J, DEG, MODE>(uv[v], cellf, cx, cy, p, tab, g[v]);
     }
 }
 
 // a3 arithmetic for V visibilities of one cell: J independent row chains per visibility (a dependent FFMA2 is
 // V J instructions away), two column chains.
-template <int J, int DEG, int MODE, int V>
-__device__ __forceinline__ void x_degrid_vis(const float2 (&uv)[V], const float (&w)[V], float2 cellf, int cx, int cy,
-                                             const XParams& p, const float* tab, const float2 (&B)[J][J], float2 (&out)[V]) {
-    float2 g[V][J];
-    x_weights_v<J, DEG, MODE, V>(uv, cellf, cx, cy, p, tab, g);
-    float2 r[V][J];
+template <typename F, int J, int DEG, int MODE, int V>
+__device__ __forceinline__ void x_degrid_vis(const C2<F> (&uv)[V], const F (&w)[V], C2<F> cellf, int cx, int cy,
+                                             const XParamsT<F>& p, const F* tab, const C2<F> (&B)[J][J], C2<F> (&out)[V]) {
+    C2<F> g[V][J];
+    x_weights_v<F, J, DEG, MODE, V>(uv, cellf, cx, cy, p, tab, g);
+    C2<F> r[V][J];
 #pragma unroll
     for (int a = 0; a < J; ++a)
 #pragma unroll
@@ -449,7 +460,7 @@ __device__ __forceinline__ void x_degrid_vis(const float2 (&uv)[V], const float 
         for (int a = 0; a < J; ++a)
 #pragma unroll
             for (int v = 0; v < V; ++v) r[v][a] = fma2(dup2(g[v][c].x), B[a][c], r[v][a]);
-    float2 acc0[V], acc1[V];
+    C2<F> acc0[V], acc1[V];
 #pragma unroll
     for (int v = 0; v < V; ++v) { acc0[v] = mul2(dup2(g[v][0].y), r[v][0]); acc1[v] = mul2(dup2(g[v][1].y), r[v][1]); }
 #pragma unroll
@@ -464,17 +475,17 @@ __device__ __forceinline__ void x_degrid_vis(const float2 (&uv)[V], const float 
 }
 
 // a4 arithmetic for V visibilities of one cell: A[a][c] += g_x[c] (g_y[a] w y), visibility by visibility per tap
-template <int J, int DEG, int MODE, int V>
-__device__ __forceinline__ void x_grid_vis(const float2 (&uv)[V], const float (&w)[V], const float2 (&yv)[V], float2 cellf,
-                                           int cx, int cy, const XParams& p, const float* tab, float2 (&A)[J][J]) {
-    float2 g[V][J];
-    x_weights_v<J, DEG, MODE, V>(uv, cellf, cx, cy, p, tab, g);
-    float2 z[V];
+template <typename F, int J, int DEG, int MODE, int V>
+__device__ __forceinline__ void x_grid_vis(const C2<F> (&uv)[V], const F (&w)[V], const C2<F> (&yv)[V], C2<F> cellf,
+                                           int cx, int cy, const XParamsT<F>& p, const F* tab, C2<F> (&A)[J][J]) {
+    C2<F> g[V][J];
+    x_weights_v<F, J, DEG, MODE, V>(uv, cellf, cx, cy, p, tab, g);
+    C2<F> z[V];
 #pragma unroll
     for (int v = 0; v < V; ++v) z[v] = mul2(dup2(w[v]), yv[v]);
 #pragma unroll
     for (int a = 0; a < J; ++a) {
-        float2 q[V];
+        C2<F> q[V];
 #pragma unroll
         for (int v = 0; v < V; ++v) q[v] = mul2(dup2(g[v][a].y), z[v]);
 #pragma unroll
@@ -514,27 +525,41 @@ __device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gsrc, uint3
                  ::"r"(smem_u32(smem_dst)), "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-__device__ __forceinline__ float2 lds_v2(uint32_t a) {
+template <typename F> __device__ __forceinline__ C2<F> lds_v2(uint32_t a);
+template <> __device__ __forceinline__ float2 lds_v2<float>(uint32_t a) {
     float2 v;
     asm volatile("ld.volatile.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(a) : "memory");
+    return v;
+}
+template <> __device__ __forceinline__ double2 lds_v2<double>(uint32_t a) {
+    double2 v;
+    asm volatile("ld.volatile.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a) : "memory");
     return v;
 }
 __device__ __forceinline__ void sts_v2(uint32_t a, float2 v) {
     asm volatile("st.volatile.shared.v2.f32 [%0], {%1, %2};" ::"r"(a), "f"(v.x), "f"(v.y) : "memory");
 }
+__device__ __forceinline__ void sts_v2(uint32_t a, double2 v) {
+    asm volatile("st.volatile.shared.v2.f64 [%0], {%1, %2};" ::"r"(a), "d"(v.x), "d"(v.y) : "memory");
+}
+// grid[idx] += v: one 8-byte vector reduction for complex64, two fp64 reductions for complex128
+__device__ __forceinline__ void atomic_add2(float2* addr, float2 v) { atomicAdd(addr, v); }
+__device__ __forceinline__ void atomic_add2(double2* addr, double2 v) { atomicAdd(&addr->x, v.x); atomicAdd(&addr->y, v.y); }
 
 // NY = number of complex64 native-order vectors streamed next to the records: 0 (degridding), 1 (gridding: y),
 // 2 (degridding + residual norm of the ADMM step: s, y), 3 (gridding of the ADMM step: v, s, y)
-template <int CH, int NY> struct RingCfg {
-    static constexpr int REC = CH * REC_BYTES, Y = CH * 256;
+template <typename F, int CH, int NY> struct RingCfg {
+    static constexpr int REC_B = REC_FLOATS * (int)sizeof(F), Y_B = 64 * (int)sizeof(F);   // bytes per iteration
+    static constexpr int REC = CH * REC_B, Y = CH * Y_B;
     static constexpr int STAGE = REC + NY * Y;
 };
 
 // warps per CTA: 4; 8 for the shared-memory-table kernels (MODE 2), so that one copy of the table serves more warps
 __host__ __device__ constexpr int x_warps(int MODE) { return MODE == 2 ? 8 : 4; }
 
-template <int J, int CH, int S, int NY, int NW = 4> struct XSmem {
-    static constexpr int WARP_BYTES = XCfg<J>::REGION_BYTES + S * RingCfg<CH, NY>::STAGE;
+template <typename F, int J, int CH, int S, int NY, int NW = 4> struct XSmem {
+    static constexpr int BOX_BYTES = XCfg<J>::REGION_BYTES * ((int)sizeof(F) / 4);
+    static constexpr int WARP_BYTES = BOX_BYTES + S * RingCfg<F, CH, NY>::STAGE;
     static constexpr int BARS = S + 1;                   // per warp: the box + the ring stages
     static constexpr size_t TOTAL = (size_t)NW * WARP_BYTES + NW * BARS * sizeof(uint64_t);   // (+ the table, MODE 2)
 };
@@ -542,18 +567,18 @@ template <int J, int CH, int S, int NY, int NW = 4> struct XSmem {
 // one lane: start the copies of chunk c (iterations [c CH, c CH + n)) of the item into `stage`.
 // (No proxy fence: the stage was only READ through the generic proxy, and those reads are ordered
 // before this call by the __syncwarp() that precedes it.)
-template <int CH, int NY>
-__device__ __forceinline__ void ring_issue(unsigned char* ring, uint64_t* rbar, int stage, const XParams& p,
-                                           const float2* y0, const float2* y1, const float2* y2, unsigned iter0, int c, int T) {
-    typedef RingCfg<CH, NY> R;
+template <typename F, int CH, int NY>
+__device__ __forceinline__ void ring_issue(unsigned char* ring, uint64_t* rbar, int stage, const XParamsT<F>& p,
+                                           const C2<F>* y0, const C2<F>* y1, const C2<F>* y2, unsigned iter0, int c, int T) {
+    typedef RingCfg<F, CH, NY> R;
     const int n = min(CH, T - c * CH);
     const size_t i0 = (size_t)iter0 + (size_t)c * CH;
     unsigned char* st = ring + stage * R::STAGE;
-    mbar_expect_tx(rbar + stage, (uint32_t)(n * (REC_BYTES + NY * 256)));
-    bulk_g2s(st, p.rec + i0 * REC_FLOATS, (uint32_t)(n * REC_BYTES), rbar + stage);
-    if (NY >= 1) bulk_g2s(st + R::REC, y0 + i0 * 32, (uint32_t)(n * 256), rbar + stage);
-    if (NY >= 2) bulk_g2s(st + R::REC + R::Y, y1 + i0 * 32, (uint32_t)(n * 256), rbar + stage);
-    if (NY >= 3) bulk_g2s(st + R::REC + 2 * R::Y, y2 + i0 * 32, (uint32_t)(n * 256), rbar + stage);
+    mbar_expect_tx(rbar + stage, (uint32_t)(n * (R::REC_B + NY * R::Y_B)));
+    bulk_g2s(st, p.rec + i0 * REC_FLOATS, (uint32_t)(n * R::REC_B), rbar + stage);
+    if (NY >= 1) bulk_g2s(st + R::REC, y0 + i0 * 32, (uint32_t)(n * R::Y_B), rbar + stage);
+    if (NY >= 2) bulk_g2s(st + R::REC + R::Y, y1 + i0 * 32, (uint32_t)(n * R::Y_B), rbar + stage);
+    if (NY >= 3) bulk_g2s(st + R::REC + 2 * R::Y, y2 + i0 * 32, (uint32_t)(n * R::Y_B), rbar + stage);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -562,24 +587,25 @@ __device__ __forceinline__ void ring_issue(unsigned char* ring, uint64_t* rbar, 
 // per batch every lane loads its cell's J x J patch into registers and then runs its unit's
 // visibilities out of registers.  HBM per slot: uv 8 + w 4 read, y 8 written (native order).
 // FUSE = 1 (f1): additionally streams s and y and accumulates ||v + s - y||^2 over the real slots into *p.norm2 (fp64).
-template <int J, int DEG, int MODE, int CH, int S, int FUSE = 0>
-__global__ void __launch_bounds__(x_warps(MODE) * 32, MODE == 2 ? 1 : (J <= 6 ? (XVD == 1 ? 4 : (XVD == 2 ? 3 : 2)) : 1))
-degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float2* __restrict__ y) {
+template <typename F, int J, int DEG, int MODE, int CH, int S, int FUSE = 0>
+__global__ void __launch_bounds__(x_warps(MODE) * 32, (MODE == 2 || sizeof(F) == 8) ? 1 : (J <= 6 ? (XVD == 1 ? 4 : (XVD == 2 ? 3 : 2)) : 1))
+degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParamsT<F> p, C2<F>* __restrict__ y) {
     typedef XCfg<J> Cfg;
+    constexpr int XVK = sizeof(F) == 4 ? XVD : 1;        // visibilities per trip (complex128: 1, registers)
     constexpr int NY = FUSE ? 2 : 0;
-    typedef RingCfg<CH, NY> R;
+    typedef RingCfg<F, CH, NY> R;
     constexpr int NW = x_warps(MODE);
-    typedef XSmem<J, CH, S, NY, NW> SM;
+    typedef XSmem<F, J, CH, S, NY, NW> SM;
     constexpr int BOXW = Cfg::BOXW, BOXH = Cfg::BOXH, XOFF = Cfg::XOFF;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    float2* tile = reinterpret_cast<float2*>(smem_raw + warp * SM::WARP_BYTES);
-    unsigned char* ring = smem_raw + warp * SM::WARP_BYTES + Cfg::REGION_BYTES;
+    C2<F>* tile = reinterpret_cast<C2<F>*>(smem_raw + warp * SM::WARP_BYTES);
+    unsigned char* ring = smem_raw + warp * SM::WARP_BYTES + SM::BOX_BYTES;
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + NW * SM::WARP_BYTES) + warp * SM::BARS;
     uint64_t* rbar = bar + 1;
-    const float* tab = p.table;
+    const F* tab = p.table;
     if (MODE == 2) {                                    // the CTA's copy of the pre-sampled table (the only CTA-wide step)
-        float* ts = reinterpret_cast<float*>(smem_raw + SM::TOTAL);
+        F* ts = reinterpret_cast<F*>(smem_raw + SM::TOTAL);
         for (int i = threadIdx.x; i < p.table_len; i += NW * 32) ts[i] = __ldg(p.table + i);
         __syncthreads();
         tab = ts;
@@ -609,12 +635,12 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
         if (lane == 0) {
             if (interior) {
                 fence_proxy_async();
-                mbar_expect_tx(bar, (uint32_t)(sizeof(float2) * BOXW * BOXH));
+                mbar_expect_tx(bar, (uint32_t)(sizeof(C2<F>) * BOXW * BOXH));
                 tma_load_2d(tile, &tmap, 2 * bx0, by0, bar);
             }
             int st = stage;
             for (int c = 0; c < S && c < nch; ++c) {
-                ring_issue<CH, NY>(ring, rbar, st, p, p.s_in, p.yobs, nullptr, it.iter0, c, T);
+                ring_issue<F, CH, NY>(ring, rbar, st, p, p.s_in, p.yobs, nullptr, it.iter0, c, T);
                 st = st + 1 == S ? 0 : st + 1;
             }
         }
@@ -631,9 +657,9 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
         }
         int left = T;                                   // iterations of the item not yet started
         int rem = 0;                                    // iterations left in the current chunk
-        const float* rp = nullptr;                      // this lane's view of the current record
-        const float2* sp = nullptr;                     // FUSE: this lane's s of the current slot (y is CH*32 entries further)
-        float2* yout = y + (size_t)it.iter0 * 32 + lane;
+        const F* rp = nullptr;                      // this lane's view of the current record
+        const C2<F>* sp = nullptr;                     // FUSE: this lane's s of the current slot (y is CH*32 entries further)
+        C2<F>* yout = y + (size_t)it.iter0 * 32 + lane;
         for (int b = it.begin; b < it.end; ++b) {
             const uint2 h = hn;
             const unsigned lw = lwn;
@@ -646,10 +672,10 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
             const int cnt = (int)(lw >> 16);
             const int ly = (lw >> 5) & 15, lx = lw & 31;
             const int cx = it.x0 + lx - p.Kh, cy = it.y0 + ly - p.Kh;       // cell = floor(u'), floor(v')
-            const float2 cellf = make_float2((float)cx, (float)cy);
-            float2 B[J][J];
+            const C2<F> cellf = mk2<F>((F)cx, (F)cy);
+            C2<F> B[J][J];
             {
-                const float2* src = tile + ly * BOXW + lx + XOFF;
+                const C2<F>* src = tile + ly * BOXW + lx + XOFF;
 #pragma unroll
                 for (int a = 0; a < J; ++a)
 #pragma unroll
@@ -662,48 +688,48 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
                     mbar_wait(rbar + stage, ring_phase);
                     rem = min(CH, left);
                     left -= rem;
-                    rp = reinterpret_cast<const float*>(ring + stage * R::STAGE) + lane;
-                    if (FUSE) sp = reinterpret_cast<const float2*>(ring + stage * R::STAGE + R::REC) + lane;
+                    rp = reinterpret_cast<const F*>(ring + stage * R::STAGE) + lane;
+                    if (FUSE) sp = reinterpret_cast<const C2<F>*>(ring + stage * R::STAGE + R::REC) + lane;
                 }
                 const int seg = min(rem, n_iter - i);
                 int k = 0;
 #pragma unroll 1
-                for (; k + XVD <= seg; k += XVD) {            // XVD visibilities per trip: XVD interleaved dependency graphs
-                    float2 uvk[XVD], o[XVD];
-                    float wk[XVD];
+                for (; k + XVK <= seg; k += XVK) {            // XVK visibilities per trip: XVK interleaved dependency graphs
+                    C2<F> uvk[XVK], o[XVK];
+                    F wk[XVK];
 #pragma unroll
-                    for (int v = 0; v < XVD; ++v) {
-                        uvk[v] = *reinterpret_cast<const float2*>(rp + v * REC_FLOATS + lane);
+                    for (int v = 0; v < XVK; ++v) {
+                        uvk[v] = *reinterpret_cast<const C2<F>*>(rp + v * REC_FLOATS + lane);
                         wk[v] = rp[v * REC_FLOATS + 64];
                     }
-                    rp += XVD * REC_FLOATS;
-                    x_degrid_vis<J, DEG, MODE, XVD>(uvk, wk, cellf, cx, cy, p, tab, B, o);
+                    rp += XVK * REC_FLOATS;
+                    x_degrid_vis<F, J, DEG, MODE, XVK>(uvk, wk, cellf, cx, cy, p, tab, B, o);
 #pragma unroll
-                    for (int v = 0; v < XVD; ++v) yout[v * 32] = o[v];
-                    yout += XVD * 32;
+                    for (int v = 0; v < XVK; ++v) yout[v * 32] = o[v];
+                    yout += XVK * 32;
                     if (FUSE) {
 #pragma unroll
-                        for (int v = 0; v < XVD; ++v)
+                        for (int v = 0; v < XVK; ++v)
                             if (i + k + v < cnt) {                          // a real slot: d = v + s - y
-                                const float2 sv = sp[v * 32], yv = sp[CH * 32 + v * 32];
-                                const float dx = (o[v].x + sv.x) - yv.x, dy = (o[v].y + sv.y) - yv.y;
+                                const C2<F> sv = sp[v * 32], yv = sp[CH * 32 + v * 32];
+                                const F dx = (o[v].x + sv.x) - yv.x, dy = (o[v].y + sv.y) - yv.y;
                                 nacc += (double)(dx * dx + dy * dy);
                             }
-                        sp += XVD * 32;
+                        sp += XVK * 32;
                     }
                 }
-                for (; XVD > 1 && k < seg; ++k) {            // tail of the segment, one visibility at a time
-                    const float2 uv1[1] = {*reinterpret_cast<const float2*>(rp + lane)};
-                    const float w1[1] = {rp[64]};
-                    float2 o1[1];
+                for (; XVK > 1 && k < seg; ++k) {            // tail of the segment, one visibility at a time
+                    const C2<F> uv1[1] = {*reinterpret_cast<const C2<F>*>(rp + lane)};
+                    const F w1[1] = {rp[64]};
+                    C2<F> o1[1];
                     rp += REC_FLOATS;
-                    x_degrid_vis<J, DEG, MODE, 1>(uv1, w1, cellf, cx, cy, p, tab, B, o1);
+                    x_degrid_vis<F, J, DEG, MODE, 1>(uv1, w1, cellf, cx, cy, p, tab, B, o1);
                     *yout = o1[0];
                     yout += 32;
                     if (FUSE) {
                         if (i + k < cnt) {
-                            const float2 sv = sp[0], yv = sp[CH * 32];
-                            const float dx = (o1[0].x + sv.x) - yv.x, dy = (o1[0].y + sv.y) - yv.y;
+                            const C2<F> sv = sp[0], yv = sp[CH * 32];
+                            const F dx = (o1[0].x + sv.x) - yv.x, dy = (o1[0].y + sv.y) - yv.y;
                             nacc += (double)(dx * dx + dy * dy);
                         }
                         sp += 32;
@@ -714,7 +740,7 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
                 if (rem == 0) {                                             // chunk consumed: refill its stage
                     __syncwarp();
                     if (cnext < nch) {
-                        if (lane == 0) ring_issue<CH, NY>(ring, rbar, stage, p, p.s_in, p.yobs, nullptr, it.iter0, cnext, T);
+                        if (lane == 0) ring_issue<F, CH, NY>(ring, rbar, stage, p, p.s_in, p.yobs, nullptr, it.iter0, cnext, T);
                         ++cnext;
                     }
                     if (++stage == S) { stage = 0; ring_phase ^= 1; }
@@ -739,25 +765,25 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, float
 // one band meet there).
 // FUSE = 1 (f1): y is v = Phi x; s and the measurements are streamed too, the gridded vector z = v - r + s_new is formed
 // slot by slot (never stored) and s_new is written to p.s_out (kernels.cuh: admm_update_kernel has the formulas).
-template <int J, int DEG, int MODE, int CH, int S, int FUSE = 0>
-__global__ void __launch_bounds__(x_warps(MODE) * 32, MODE == 2 ? 1 : (J <= 6 ? 4 : 1))
-grid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, const float2* __restrict__ y) {
+template <typename F, int J, int DEG, int MODE, int CH, int S, int FUSE = 0>
+__global__ void __launch_bounds__(x_warps(MODE) * 32, (MODE == 2 || sizeof(F) == 8) ? 1 : (J <= 6 ? 4 : 1))
+grid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParamsT<F> p, const C2<F>* __restrict__ y) {
     typedef XCfg<J> Cfg;
     constexpr int NY = FUSE ? 3 : 1;
-    typedef RingCfg<CH, NY> R;
-    constexpr int XVG = J == 4 ? XVG4 : XVG6;            // visibilities per trip
+    typedef RingCfg<F, CH, NY> R;
+    constexpr int XVG = sizeof(F) == 8 ? 1 : (J == 4 ? XVG4 : XVG6);   // visibilities per trip
     constexpr int NW = x_warps(MODE);
-    typedef XSmem<J, CH, S, NY, NW> SM;
+    typedef XSmem<F, J, CH, S, NY, NW> SM;
     constexpr int BOXW = Cfg::BOXW, BOXH = Cfg::BOXH, XOFF = Cfg::XOFF;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    float2* tile = reinterpret_cast<float2*>(smem_raw + warp * SM::WARP_BYTES);
-    unsigned char* ring = smem_raw + warp * SM::WARP_BYTES + Cfg::REGION_BYTES;
+    C2<F>* tile = reinterpret_cast<C2<F>*>(smem_raw + warp * SM::WARP_BYTES);
+    unsigned char* ring = smem_raw + warp * SM::WARP_BYTES + SM::BOX_BYTES;
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + NW * SM::WARP_BYTES) + warp * SM::BARS;
     uint64_t* rbar = bar + 1;
-    const float* tab = p.table;
+    const F* tab = p.table;
     if (MODE == 2) {                                    // the CTA's copy of the pre-sampled table (the only CTA-wide step)
-        float* ts = reinterpret_cast<float*>(smem_raw + SM::TOTAL);
+        F* ts = reinterpret_cast<F*>(smem_raw + SM::TOTAL);
         for (int i = threadIdx.x; i < p.table_len; i += NW * 32) ts[i] = __ldg(p.table + i);
         __syncthreads();
         tab = ts;
@@ -769,16 +795,16 @@ grid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, const f
     __syncwarp();
     uint32_t ring_phase = 0;
     int stage = 0;
-    const float oma = FUSE ? (float)(1.0 - admm_alpha(*p.norm2, p.eps)) : 0.f, vrho = (float)p.varrho;
+    const F oma = FUSE ? (F)(1.0 - admm_alpha(*p.norm2, p.eps)) : (F)0, vrho = (F)p.varrho;
     // one slot of the fused ADMM step: (v, s, y) -> z = v - r + s_new, s_new stored; padding slots give 0
-    auto admm_slot = [&](const float2* q, bool real_slot, float2* sdst) -> float2 {
-        float2 z = make_float2(0.f, 0.f), sn = z;
+    auto admm_slot = [&](const C2<F>* q, bool real_slot, C2<F>* sdst) -> C2<F> {
+        C2<F> z = mk2<F>((F)0, (F)0), sn = z;
         if (real_slot) {
-            const float2 vv = q[0], sv = q[CH * 32], yv = q[2 * CH * 32];
-            const float dx = (vv.x + sv.x) - yv.x, dy = (vv.y + sv.y) - yv.y;
-            const float vrx = oma * dx - sv.x, vry = oma * dy - sv.y;
-            sn = make_float2(sv.x + vrho * vrx, sv.y + vrho * vry);
-            z = make_float2(vrx + sn.x, vry + sn.y);
+            const C2<F> vv = q[0], sv = q[CH * 32], yv = q[2 * CH * 32];
+            const F dx = (vv.x + sv.x) - yv.x, dy = (vv.y + sv.y) - yv.y;
+            const F vrx = oma * dx - sv.x, vry = oma * dy - sv.y;
+            sn = mk2<F>(sv.x + vrho * vrx, sv.y + vrho * vry);
+            z = mk2<F>(vrx + sn.x, vry + sn.y);
         }
         *sdst = sn;
         return z;
@@ -796,19 +822,19 @@ grid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, const f
         if (lane == 0) {
             int st = stage;
             for (int c = 0; c < S && c < nch; ++c) {
-                ring_issue<CH, NY>(ring, rbar, st, p, y, p.s_in, p.yobs, it.iter0, c, T);
+                ring_issue<F, CH, NY>(ring, rbar, st, p, y, p.s_in, p.yobs, it.iter0, c, T);
                 st = st + 1 == S ? 0 : st + 1;
             }
         }
         int cnext = S;
         if (lane == 0) bulk_wait_group_read0();         // the previous item's box reduction has read the box
         __syncwarp();
-        for (int i = lane; i < BOXW * BOXH; i += 32) tile[i] = make_float2(0.f, 0.f);
+        for (int i = lane; i < BOXW * BOXH; i += 32) tile[i] = mk2<F>((F)0, (F)0);
         __syncwarp();
-        float2* sout = FUSE ? p.s_out + (size_t)it.iter0 * 32 + lane : nullptr;
+        C2<F>* sout = FUSE ? p.s_out + (size_t)it.iter0 * 32 + lane : nullptr;
         int left = T, rem = 0;
-        const float* rp = nullptr;
-        const float2* yp = nullptr;
+        const F* rp = nullptr;
+        const C2<F>* yp = nullptr;
         for (int b = it.begin; b < it.end; ++b) {
             const uint2 h = hn;
             const unsigned lw = lwn;
@@ -822,72 +848,72 @@ grid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, const f
             const int cnt = (int)(lw >> 16);
             const int ly = (lw >> 5) & 15, lx = lw & 31;
             const int cx = it.x0 + lx - p.Kh, cy = it.y0 + ly - p.Kh;
-            const float2 cellf = make_float2((float)cx, (float)cy);
-            float2 A[J][J];
+            const C2<F> cellf = mk2<F>((F)cx, (F)cy);
+            C2<F> A[J][J];
 #pragma unroll
             for (int a = 0; a < J; ++a)
 #pragma unroll
-                for (int c = 0; c < J; ++c) A[a][c] = make_float2(0.f, 0.f);
+                for (int c = 0; c < J; ++c) A[a][c] = mk2<F>((F)0, (F)0);
 
             for (int i = 0; i < n_iter;) {
                 if (rem == 0) {
                     mbar_wait(rbar + stage, ring_phase);
                     rem = min(CH, left);
                     left -= rem;
-                    rp = reinterpret_cast<const float*>(ring + stage * R::STAGE) + lane;
-                    yp = reinterpret_cast<const float2*>(ring + stage * R::STAGE + R::REC) + lane;
+                    rp = reinterpret_cast<const F*>(ring + stage * R::STAGE) + lane;
+                    yp = reinterpret_cast<const C2<F>*>(ring + stage * R::STAGE + R::REC) + lane;
                 }
                 const int seg = min(rem, n_iter - i);
                 int live = cnt - i;                                         // slots of this segment that hold a visibility
                 int k = 0;
 #pragma unroll 1
                 for (; k + XVG <= seg; k += XVG, live -= XVG) {
-                    float2 uvk[XVG], yk[XVG];
-                    float wk[XVG];
+                    C2<F> uvk[XVG], yk[XVG];
+                    F wk[XVG];
 #pragma unroll
                     for (int v = 0; v < XVG; ++v) {
-                        uvk[v] = *reinterpret_cast<const float2*>(rp + v * REC_FLOATS + lane);
+                        uvk[v] = *reinterpret_cast<const C2<F>*>(rp + v * REC_FLOATS + lane);
                         wk[v] = rp[v * REC_FLOATS + 64];
                         if (FUSE) {
                             yk[v] = admm_slot(yp + v * 32, live > v, sout + v * 32);
                         } else {
                             yk[v] = yp[v * 32];
-                            if (live <= v) yk[v] = make_float2(0.f, 0.f);   // padding slot: whatever y holds there is ignored
+                            if (live <= v) yk[v] = mk2<F>((F)0, (F)0);   // padding slot: whatever y holds there is ignored
                         }
                     }
                     rp += XVG * REC_FLOATS;
                     yp += XVG * 32;
                     if (FUSE) sout += XVG * 32;
-                    x_grid_vis<J, DEG, MODE, XVG>(uvk, wk, yk, cellf, cx, cy, p, tab, A);
+                    x_grid_vis<F, J, DEG, MODE, XVG>(uvk, wk, yk, cellf, cx, cy, p, tab, A);
                 }
                 for (; XVG > 1 && k < seg; ++k, --live) {
-                    const float2 uv1[1] = {*reinterpret_cast<const float2*>(rp + lane)};
-                    const float w1[1] = {rp[64]};
-                    float2 y1[1];
+                    const C2<F> uv1[1] = {*reinterpret_cast<const C2<F>*>(rp + lane)};
+                    const F w1[1] = {rp[64]};
+                    C2<F> y1[1];
                     if (FUSE) {
                         y1[0] = admm_slot(yp, live > 0, sout);
                         sout += 32;
                     } else {
                         y1[0] = *yp;
-                        if (live <= 0) y1[0] = make_float2(0.f, 0.f);
+                        if (live <= 0) y1[0] = mk2<F>((F)0, (F)0);
                     }
                     rp += REC_FLOATS;
                     yp += 32;
-                    x_grid_vis<J, DEG, MODE, 1>(uv1, w1, y1, cellf, cx, cy, p, tab, A);
+                    x_grid_vis<F, J, DEG, MODE, 1>(uv1, w1, y1, cellf, cx, cy, p, tab, A);
                 }
                 i += seg;
                 rem -= seg;
                 if (rem == 0) {
                     __syncwarp();
                     if (cnext < nch) {
-                        if (lane == 0) ring_issue<CH, NY>(ring, rbar, stage, p, y, p.s_in, p.yobs, it.iter0, cnext, T);
+                        if (lane == 0) ring_issue<F, CH, NY>(ring, rbar, stage, p, y, p.s_in, p.yobs, it.iter0, cnext, T);
                         ++cnext;
                     }
                     if (++stage == S) { stage = 0; ring_phase ^= 1; }
                 }
             }
             // ---- flush the accumulators into the warp's box; idle lanes (no unit) stay out
-            float2* dst = tile + ly * BOXW + lx + XOFF;
+            C2<F>* dst = tile + ly * BOXW + lx + XOFF;
             if (!dup) {
                 // One read-modify-write per tap.  In step (a, c) the lanes touch distinct addresses (distinct
                 // cells); the footprints of different lanes overlap ACROSS steps, so step s+1 must see step s.
@@ -902,8 +928,8 @@ grid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, const f
                     for (int a = 0; a < J; ++a)
 #pragma unroll
                         for (int c = 0; c < J; ++c) {
-                            const uint32_t ad = da + (uint32_t)(a * BOXW + c) * 8u;
-                            sts_v2(ad, add2(lds_v2(ad), A[a][c]));
+                            const uint32_t ad = da + (uint32_t)(a * BOXW + c) * (uint32_t)sizeof(C2<F>);
+                            sts_v2(ad, add2(lds_v2<F>(ad), A[a][c]));
                         }
                 }
                 __syncwarp();
@@ -926,7 +952,7 @@ grid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, const f
         __syncwarp();
         const int bx0 = it.x0 - (J / 2 - 1) - XOFF, by0 = it.y0 - (J / 2 - 1);
         const bool interior = bx0 >= 0 && by0 >= 0 && bx0 + BOXW <= p.K && by0 + BOXH <= p.K;
-        if (interior) {
+        if (interior && sizeof(F) == 4) {                // (no fp64 add in the TMA reduction: complex128 uses the loop below)
             if (lane == 0) {
                 fence_proxy_async();
                 tma_reduce_add_2d(&tmap, 2 * bx0, by0, tile);
@@ -934,10 +960,10 @@ grid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParams p, const f
             }
         } else {
             for (int i = lane; i < BOXW * BOXH; i += 32) {
-                const float2 v = tile[i];
-                if (v.x != 0.f || v.y != 0.f) {
+                const C2<F> v = tile[i];
+                if (v.x != (F)0 || v.y != (F)0) {
                     const int r = wrap_idx(by0 + i / BOXW, p.K, p.kmask), c = wrap_idx(bx0 + i % BOXW, p.K, p.kmask);
-                    atomicAdd(p.grid + (long long)r * p.K + c, v);
+                    atomic_add2(p.grid + (long long)r * p.K + c, v);
                 }
             }
         }

@@ -193,9 +193,10 @@ template <typename R, int J, int DEG> int launch_grid_t(purify_op* op, const voi
     return PURIFY_OK;
 }
 
-pk::XParams make_xparams(const purify_op* op, bool caller_order) {
-    pk::XParams p;
-    p.grid = (float2*)op->grid;
+template <typename F> pk::XParamsT<F> make_xparams(const purify_op* op) {
+    typedef typename pk::Cplx<F>::type F2;
+    pk::XParamsT<F> p;
+    p.grid = (F2*)op->grid;
     p.K = op->K; p.Kh = op->K / 2;
     p.kmask = (op->K & (op->K - 1)) == 0 ? op->K - 1 : 0;
     p.items = op->x_items;
@@ -203,11 +204,10 @@ pk::XParams make_xparams(const purify_op* op, bool caller_order) {
     p.counter = op->x_counter;
     p.bhdr = op->x_bhdr;
     p.blane = op->x_blane;
-    p.rec = (const float*)op->uv_s;
-    (void)caller_order;
-    memcpy(&p.coef, &op->coef32, sizeof(p.coef));
-    p.table = (const float*)op->table;
-    p.table_R = (float)op->table_R;
+    p.rec = (const F*)op->uv_s;
+    if (sizeof(F) == 4) memcpy(&p.coef, &op->coef32, sizeof(p.coef)); else memcpy(&p.coef, &op->coef64, sizeof(p.coef));
+    p.table = (const F*)op->table;
+    p.table_R = (F)op->table_R;
     p.table_len = op->table_len;
     p.s_in = nullptr; p.yobs = nullptr; p.s_out = nullptr; p.norm2 = op->scal_ws; p.eps = 0.0; p.varrho = 0.0;
     return p;
@@ -249,33 +249,35 @@ constexpr size_t X_TABLE_SMEM_MAX = 64 * 1024;
 
 struct AdmmArgs { const void* y_obs; void* s; double eps, varrho; };
 
-template <int J, int DEG, int MODE, int CH, int S, int FUSE = 0>
+template <typename F, int J, int DEG, int MODE, int CH, int S, int FUSE = 0>
 int launch_degrid_x_m(purify_op* op, void* y, size_t extra_smem, cudaStream_t st, const AdmmArgs* aa = nullptr) {
+    typedef typename pk::Cplx<F>::type F2;
     constexpr int NW = pk::x_warps(MODE);
-    const size_t smem = pk::XSmem<J, CH, S, FUSE ? 2 : 0, NW>::TOTAL + extra_smem;
-    pk::XParams p = make_xparams(op, false);
-    if (aa) { p.s_in = (const float2*)aa->s; p.yobs = (const float2*)aa->y_obs; p.s_out = (float2*)aa->s; p.eps = aa->eps; p.varrho = aa->varrho; }
+    const size_t smem = pk::XSmem<F, J, CH, S, FUSE ? 2 : 0, NW>::TOTAL + extra_smem;
+    pk::XParamsT<F> p = make_xparams<F>(op);
+    if (aa) { p.s_in = (const F2*)aa->s; p.yobs = (const F2*)aa->y_obs; p.s_out = (F2*)aa->s; p.eps = aa->eps; p.varrho = aa->varrho; }
     CK(cudaMemsetAsync(op->x_counter, 0, sizeof(unsigned), st));
     int g = 0, rc;
-    auto kern = pk::degrid_x_kernel<J, DEG, MODE, CH, S, FUSE>;
+    auto kern = pk::degrid_x_kernel<F, J, DEG, MODE, CH, S, FUSE>;
     if ((rc = x_grid_size(kern, NW * 32, smem, op->n_items, NW, &g))) return rc;
-    kern<<<g, NW * 32, smem, st>>>(op->tmap_x, p, (float2*)y);
+    kern<<<g, NW * 32, smem, st>>>(op->tmap_x, p, (F2*)y);
     op->launches++;
     CK(cudaGetLastError());
     return PURIFY_OK;
 }
 
-template <int J, int DEG, int MODE, int CH, int S, int FUSE = 0>
+template <typename F, int J, int DEG, int MODE, int CH, int S, int FUSE = 0>
 int launch_grid_x_m(purify_op* op, const void* y, size_t extra_smem, cudaStream_t st, const AdmmArgs* aa = nullptr) {
+    typedef typename pk::Cplx<F>::type F2;
     constexpr int NW = pk::x_warps(MODE);
-    const size_t smem = pk::XSmem<J, CH, S, FUSE ? 3 : 1, NW>::TOTAL + extra_smem;
-    pk::XParams p = make_xparams(op, false);
-    if (aa) { p.s_in = (const float2*)aa->s; p.yobs = (const float2*)aa->y_obs; p.s_out = (float2*)aa->s; p.eps = aa->eps; p.varrho = aa->varrho; }
+    const size_t smem = pk::XSmem<F, J, CH, S, FUSE ? 3 : 1, NW>::TOTAL + extra_smem;
+    pk::XParamsT<F> p = make_xparams<F>(op);
+    if (aa) { p.s_in = (const F2*)aa->s; p.yobs = (const F2*)aa->y_obs; p.s_out = (F2*)aa->s; p.eps = aa->eps; p.varrho = aa->varrho; }
     CK(cudaMemsetAsync(op->x_counter, 0, sizeof(unsigned), st));
     int g = 0, rc;
-    auto kern = pk::grid_x_kernel<J, DEG, MODE, CH, S, FUSE>;
+    auto kern = pk::grid_x_kernel<F, J, DEG, MODE, CH, S, FUSE>;
     if ((rc = x_grid_size(kern, NW * 32, smem, op->n_items, NW, &g))) return rc;
-    kern<<<g, NW * 32, smem, st>>>(op->tmap_x, p, (const float2*)y);
+    kern<<<g, NW * 32, smem, st>>>(op->tmap_x, p, (const F2*)y);
     op->launches++;
     CK(cudaGetLastError());
     return PURIFY_OK;
@@ -284,17 +286,33 @@ int launch_grid_x_m(purify_op* op, const void* y, size_t extra_smem, cudaStream_
 template <int J, int DEG> int launch_degrid_x_t(purify_op* op, void* y, cudaStream_t st) {
     if (op->n_items == 0) return PURIFY_OK;
     const size_t tb = sizeof(float) * (size_t)op->table_len;
-    if (op->mode != PURIFY_KERNEL_TABLE) return launch_degrid_x_m<J, DEG, 0, X_CH_DEGRID, X_S_DEGRID>(op, y, 0, st);
-    if (tb <= X_TABLE_SMEM_MAX) return launch_degrid_x_m<J, DEG, 2, X_CH_DEGRID_T, X_S_DEGRID_T>(op, y, tb, st);
-    return launch_degrid_x_m<J, DEG, 1, X_CH_DEGRID_T, X_S_DEGRID_T>(op, y, 0, st);
+    if (op->mode != PURIFY_KERNEL_TABLE) return launch_degrid_x_m<float, J, DEG, 0, X_CH_DEGRID, X_S_DEGRID>(op, y, 0, st);
+    if (tb <= X_TABLE_SMEM_MAX) return launch_degrid_x_m<float, J, DEG, 2, X_CH_DEGRID_T, X_S_DEGRID_T>(op, y, tb, st);
+    return launch_degrid_x_m<float, J, DEG, 1, X_CH_DEGRID_T, X_S_DEGRID_T>(op, y, 0, st);
 }
 
 template <int J, int DEG> int launch_grid_x_t(purify_op* op, const void* y, cudaStream_t st) {
     if (op->n_items == 0) return PURIFY_OK;
     const size_t tb = sizeof(float) * (size_t)op->table_len;
-    if (op->mode != PURIFY_KERNEL_TABLE) return launch_grid_x_m<J, DEG, 0, X_CH_GRID, X_S_GRID>(op, y, 0, st);
-    if (tb <= X_TABLE_SMEM_MAX) return launch_grid_x_m<J, DEG, 2, X_CH_GRID_T, X_S_GRID_T>(op, y, tb, st);
-    return launch_grid_x_m<J, DEG, 1, X_CH_GRID_T, X_S_GRID_T>(op, y, 0, st);
+    if (op->mode != PURIFY_KERNEL_TABLE) return launch_grid_x_m<float, J, DEG, 0, X_CH_GRID, X_S_GRID>(op, y, 0, st);
+    if (tb <= X_TABLE_SMEM_MAX) return launch_grid_x_m<float, J, DEG, 2, X_CH_GRID_T, X_S_GRID_T>(op, y, tb, st);
+    return launch_grid_x_m<float, J, DEG, 1, X_CH_GRID_T, X_S_GRID_T>(op, y, 0, st);
+}
+
+// complex128 in the batched layout (J = 4, 6; J = 8 does not fit the register file and keeps the tile-sorted kernels):
+// same kernels instantiated for double - component-wise fp64 arithmetic, one visibility per trip, table in global memory
+constexpr int X_CH_DEGRID_D = 8, X_S_DEGRID_D = 2, X_CH_GRID_D = 4, X_S_GRID_D = 2;
+
+template <int J, int DEG> int launch_degrid_x_d(purify_op* op, void* y, cudaStream_t st) {
+    if (op->n_items == 0) return PURIFY_OK;
+    if (op->mode != PURIFY_KERNEL_TABLE) return launch_degrid_x_m<double, J, DEG, 0, X_CH_DEGRID_D, X_S_DEGRID_D>(op, y, 0, st);
+    return launch_degrid_x_m<double, J, DEG, 1, X_CH_DEGRID_D, X_S_DEGRID_D>(op, y, 0, st);
+}
+
+template <int J, int DEG> int launch_grid_x_d(purify_op* op, const void* y, cudaStream_t st) {
+    if (op->n_items == 0) return PURIFY_OK;
+    if (op->mode != PURIFY_KERNEL_TABLE) return launch_grid_x_m<double, J, DEG, 0, X_CH_GRID_D, X_S_GRID_D>(op, y, 0, st);
+    return launch_grid_x_m<double, J, DEG, 1, X_CH_GRID_D, X_S_GRID_D>(op, y, 0, st);
 }
 
 // f1, fused (complex64 batched layout, ANALYTIC weights): ring geometries that keep the occupancy of the plain kernels
@@ -304,9 +322,9 @@ int launch_degrid_fused(purify_op* op, void* v, const AdmmArgs& aa, cudaStream_t
     StageTimer t(op, PURIFY_STAGE_DEGRID, st);
     if (op->n_items == 0) return PURIFY_OK;
     switch (op->J) {
-        case 4: return launch_degrid_x_m<4, deg_c64(4), 0, X_CH_DEGRID_F, X_S_DEGRID_F, 1>(op, v, 0, st, &aa);
-        case 6: return launch_degrid_x_m<6, deg_c64(6), 0, X_CH_DEGRID_F, X_S_DEGRID_F, 1>(op, v, 0, st, &aa);
-        default: return launch_degrid_x_m<8, deg_c64(8), 0, X_CH_DEGRID_F, X_S_DEGRID_F, 1>(op, v, 0, st, &aa);
+        case 4: return launch_degrid_x_m<float, 4, deg_c64(4), 0, X_CH_DEGRID_F, X_S_DEGRID_F, 1>(op, v, 0, st, &aa);
+        case 6: return launch_degrid_x_m<float, 6, deg_c64(6), 0, X_CH_DEGRID_F, X_S_DEGRID_F, 1>(op, v, 0, st, &aa);
+        default: return launch_degrid_x_m<float, 8, deg_c64(8), 0, X_CH_DEGRID_F, X_S_DEGRID_F, 1>(op, v, 0, st, &aa);
     }
 }
 
@@ -318,14 +336,16 @@ int launch_grid_fused(purify_op* op, const void* v, const AdmmArgs& aa, cudaStre
     StageTimer t(op, PURIFY_STAGE_GRID, st);
     if (op->n_items == 0) return PURIFY_OK;
     switch (op->J) {
-        case 4: return launch_grid_x_m<4, deg_c64(4), 0, X_CH_GRID_F, X_S_GRID_F, 1>(op, v, 0, st, &aa);
-        case 6: return launch_grid_x_m<6, deg_c64(6), 0, X_CH_GRID_F, X_S_GRID_F, 1>(op, v, 0, st, &aa);
-        default: return launch_grid_x_m<8, deg_c64(8), 0, X_CH_GRID_F, X_S_GRID_F, 1>(op, v, 0, st, &aa);
+        case 4: return launch_grid_x_m<float, 4, deg_c64(4), 0, X_CH_GRID_F, X_S_GRID_F, 1>(op, v, 0, st, &aa);
+        case 6: return launch_grid_x_m<float, 6, deg_c64(6), 0, X_CH_GRID_F, X_S_GRID_F, 1>(op, v, 0, st, &aa);
+        default: return launch_grid_x_m<float, 8, deg_c64(8), 0, X_CH_GRID_F, X_S_GRID_F, 1>(op, v, 0, st, &aa);
     }
 }
 
 int launch_degrid(purify_op* op, void* y, bool caller_order, cudaStream_t st) {
     StageTimer t(op, PURIFY_STAGE_DEGRID, st);
+    if (op->batched && op->dtype == PURIFY_C128)
+        return op->J == 4 ? launch_degrid_x_d<4, deg_c128(4)>(op, y, st) : launch_degrid_x_d<6, deg_c128(6)>(op, y, st);
     if (op->batched) {
         switch (op->J) {
             case 4: return launch_degrid_x_t<4, deg_c64(4)>(op, y, st);
@@ -333,7 +353,7 @@ int launch_degrid(purify_op* op, void* y, bool caller_order, cudaStream_t st) {
             default: return launch_degrid_x_t<8, deg_c64(8)>(op, y, st);
         }
     }
-    // complex64 always uses the batched layout above; the tile-sorted kernels below serve complex128
+    // the tile-sorted kernels below serve complex128 with J = 8 (its J x J patch does not fit the register file)
     switch (op->J) {
         case 4: return launch_degrid_t<double, 4, deg_c128(4)>(op, y, caller_order, st);
         case 6: return launch_degrid_t<double, 6, deg_c128(6)>(op, y, caller_order, st);
@@ -347,6 +367,8 @@ int launch_grid(purify_op* op, const void* y, bool caller_order, cudaStream_t st
         CK(cudaMemsetAsync(op->grid, 0, csize(op) * (size_t)op->K * op->K, st));
     }
     StageTimer t(op, PURIFY_STAGE_GRID, st);
+    if (op->batched && op->dtype == PURIFY_C128)
+        return op->J == 4 ? launch_grid_x_d<4, deg_c128(4)>(op, y, st) : launch_grid_x_d<6, deg_c128(6)>(op, y, st);
     if (op->batched) {
         switch (op->J) {
             case 4: return launch_grid_x_t<4, deg_c64(4)>(op, y, st);
@@ -403,8 +425,10 @@ int launch_permute(purify_op* op, const void* in, void* out, int to_native, cuda
     StageTimer t(op, PURIFY_STAGE_PERMUTE, st);
     if (op->M_native == 0) return PURIFY_OK;
     if (!to_native && op->inv_perm) {
-        if (op->M > 0)
+        if (op->M > 0 && op->dtype == PURIFY_C64)
             pk::gather_from_native_kernel<float2><<<grid_for(op->M, 256, 148 * 32), 256, 0, st>>>((const float2*)in, (float2*)out, op->inv_perm, op->M);
+        else if (op->M > 0)
+            pk::gather_from_native_kernel<double2><<<grid_for(op->M, 256, 148 * 32), 256, 0, st>>>((const double2*)in, (double2*)out, op->inv_perm, op->M);
         op->launches++;
         CK(cudaGetLastError());
         return PURIFY_OK;
@@ -556,7 +580,9 @@ int build_bins(purify_op* op, const void* uv_dev, const void* w_dev, cudaStream_
 
 // a0 for complex64: the batched layout of batched.cuh (device radix sort on band/cell id, per-band
 // batch construction, slot fill).
+template <typename F>
 int build_bins_x(purify_op* op, const void* uv_dev, const void* w_dev, cudaStream_t st) {
+    typedef typename pk::Cplx<F>::type F2;
     const long long M = op->M;
     const int K = op->K;
     const int nbx = (K + pk::XBW - 1) / pk::XBW, nby = (K + pk::XBH - 1) / pk::XBH;
@@ -606,7 +632,7 @@ int build_bins_x(purify_op* op, const void* uv_dev, const void* w_dev, cudaStrea
     CKC(cudaMemsetAsync(nonempty, 0, sizeof(unsigned), st));
 
     if (M > 0) {
-        pk::xkey_kernel<<<grid_for(M, 256), 256, 0, st>>>((const float2*)uv_dev, M, K, nbx, keys, idx, bad);
+        pk::xkey_kernel<F><<<grid_for(M, 256), 256, 0, st>>>((const F2*)uv_dev, M, K, nbx, keys, idx, bad);
         CKC(cudaGetLastError());
         int h_bad = 0;
         CKC(cudaMemcpyAsync(&h_bad, bad, sizeof(int), cudaMemcpyDeviceToHost, st));
@@ -651,7 +677,7 @@ int build_bins_x(purify_op* op, const void* uv_dev, const void* w_dev, cudaStrea
     int rc;
     const size_t S = op->M_native > 0 ? (size_t)op->M_native : 1, NBz = op->n_batches > 0 ? op->n_batches : 1;
     // per-iteration records (uv[32] | w[32]); uv_s holds them, w_s is unused in this layout
-    if ((rc = dev_alloc(op, &op->uv_s, (size_t)pk::REC_BYTES * (S / 32 + 1)))) { cleanup(); return rc; }
+    if ((rc = dev_alloc(op, &op->uv_s, (size_t)pk::REC_FLOATS * sizeof(F) * (S / 32 + 1)))) { cleanup(); return rc; }
     if ((rc = dev_alloc(op, (void**)&op->perm, sizeof(unsigned) * S))) { cleanup(); return rc; }
     if ((rc = dev_alloc(op, (void**)&op->x_bhdr, sizeof(uint2) * NBz))) { cleanup(); return rc; }
     if ((rc = dev_alloc(op, (void**)&op->x_blane, sizeof(unsigned) * 32 * NBz))) { cleanup(); return rc; }
@@ -694,9 +720,9 @@ int build_bins_x(purify_op* op, const void* uv_dev, const void* w_dev, cudaStrea
             free5();
             CKC(e);
         }
-        pk::slot_fill_kernel<<<grid_for((long long)op->n_batches * 32, 256), 256, 0, st>>>(
-            op->x_bhdr, op->x_blane, lsrc, op->n_batches, perm0, (const float2*)uv_dev, (const float*)w_dev, K,
-            op->perm, (float*)op->uv_s);
+        pk::slot_fill_kernel<F><<<grid_for((long long)op->n_batches * 32, 256), 256, 0, st>>>(
+            op->x_bhdr, op->x_blane, lsrc, op->n_batches, perm0, (const F2*)uv_dev, (const F*)w_dev, K,
+            op->perm, (F*)op->uv_s);
         CKC(cudaGetLastError());
     }
     if (M > 0) {
@@ -771,7 +797,7 @@ int build_tmap(purify_op* op) {
             memset(&op->tmap_x, 0, sizeof(op->tmap_x));
             return PURIFY_OK;
         }
-        CUresult r = ((EncodeTiledFn)fn)(&op->tmap_x, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, op->grid, dims, strides, box, estr,
+        CUresult r = ((EncodeTiledFn)fn)(&op->tmap_x, f32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, op->grid, dims, strides, box, estr,
                                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                          CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) return fail(PURIFY_ERR_CUDA, "cuTensorMapEncodeTiled (band box) failed: CUresult %d", (int)r);
@@ -841,7 +867,9 @@ int create_impl(purify_op** out, int n, int oversample, int J, long long M, cons
     rc = dev_alloc(op, &op->grid, csize(op) * (size_t)op->K * op->K);
     if (rc) return bail(rc);
     if (dtype == PURIFY_C64) {
-        rc = build_bins_x(op, uv_dev, w_dev, st);
+        rc = build_bins_x<float>(op, uv_dev, w_dev, st);
+    } else if (J <= 6 && !(opts && opts->reserved[1])) {     // reserved[1] != 0: force the tile-sorted complex128 kernels
+        rc = build_bins_x<double>(op, uv_dev, w_dev, st);
     } else {
         rc = build_bins<double>(op, uv_dev, w_dev, st);
         op->M_native = M;
@@ -1123,7 +1151,7 @@ int purify_admm_fidelity_step(purify_op* op, const void* x_dev, const void* y_na
     RUN(ensure_ws(op, &op->y_ws, csize(op) * (size_t)Mn));
     RUN(ensure_ws(op, &op->y_ws2, csize(op) * (size_t)(Mn > op->M ? Mn : op->M)));
     RUN(ensure_ws(op, (void**)&op->scal_ws, sizeof(double)));
-    if (op->batched && op->mode == PURIFY_KERNEL_ANALYTIC && !op->admm_unfused) {
+    if (op->batched && op->dtype == PURIFY_C64 && op->mode == PURIFY_KERNEL_ANALYTIC && !op->admm_unfused) {
         // fused form: the norm is accumulated inside the degridding kernel, r / s_new / z are formed slot by slot inside
         // the gridding kernel (z is never stored); two passes over the M-sized vectors less than the unfused form below
         if (((uintptr_t)y_native_dev & 15u) || ((uintptr_t)s_native_dev & 15u))

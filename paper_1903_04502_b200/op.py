@@ -105,12 +105,13 @@ class PurifyOp:
 
     def __init__(self, n: int, J: int, uv: torch.Tensor, w: torch.Tensor | None = None, dtype: int = C64,
                  oversample: int = 2, kernel_mode: int = ANALYTIC, table_samples_per_unit: int = 0,
-                 chunk: int = 0, time_stages: bool = False, admm_unfused: bool = False):
+                 chunk: int = 0, time_stages: bool = False, admm_unfused: bool = False, tile_sorted: bool = False):
         self._L = load_library()
         self._h = C.c_void_p()
         self.n, self.K, self.J, self.dtype = int(n), 2 * int(n), int(J), int(dtype)
         opts = PurifyOpts(int(kernel_mode), int(table_samples_per_unit), int(chunk), int(bool(time_stages)))
         opts.reserved[0] = int(bool(admm_unfused))     # purify_admm_fidelity_step: separate norm / update kernels
+        opts.reserved[1] = int(bool(tile_sorted))      # complex128: the tile-sorted kernels instead of the batched layout
         M = 0 if uv is None else int(uv.shape[0])
         self.M = M
         rdt = _RDT.get(self.dtype, torch.float32)

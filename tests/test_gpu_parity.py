@@ -124,12 +124,14 @@ def test_config1_tiny(J, dtype):
 
 
 def test_config1_small_chunks():
-    """Many work items per tile (chunk 32/64) exercise the chunk flush / ragged tails."""
+    """Tile-sorted complex128 kernels (the default for J = 8, forced here for J = 4 and 6): many work items per tile
+    (chunk 32 / 96) exercise the chunk flush / ragged tails."""
     cfg, x, uv, w = synth.make_problem(1)
     w = synth.rng_for(1, 1).uniform(0.5, 1.5, size=len(uv))
-    for chunk in (32, 96):
-        info = run_all_checks(x, uv, w, 4, "c128", chunk=chunk)
-        assert info["n_items"] > info["n_tiles_nonempty"]
+    for J, chunk in ((4, 32), (4, 96), (6, 64)):
+        info = run_all_checks(x, uv, w, J, "c128", chunk=chunk, tile_sorted=True)
+        assert info["layout"] == 0 and info["n_items"] > info["n_tiles_nonempty"]
+    assert run_all_checks(x, uv, w, 4, "c128")["layout"] == 1        # default: the batched layout
 
 
 # ------------------------------------------------------------------ config 2
