@@ -20,7 +20,7 @@
  *   dtype   PURIFY_C64 : x, y complex64,  uv and w float32.   PURIFY_C128: complex128 / float64.
  *   order   "caller order" = the order of uv at create.  "native order" = the library's own order, a
  *           vector of M_native >= M entries (purify_op_info): native[i] = caller[perm[i]] with perm
- *           from purify_op_permutation(); perm[i] = 0xFFFFFFFF marks a PADDING entry (complex64
+ *           from purify_op_permutation(); perm[i] = 0xFFFFFFFF marks a PADDING entry (batched
  *           layout only): purify_degrid_native writes 0 there, purify_grid_native ignores it.
  *   memory  "_dev" pointers are CUDA device pointers on the current device, "_host" pointers are
  *           host pointers (pinned memory recommended).  The caller owns every buffer it passes; the
@@ -64,7 +64,7 @@ typedef struct {
                                    (BASELINE.json configs[4]); paper used 2e5.
                                    T[i] = g(i/R), i = 0..R*J/2+1, lookup T[floor(|d| R + 1/2)].      */
     int chunk;                  /* complex128 (tile-sorted layout): visibilities per work item (CTA); default 4096.
-                                   Ignored by the complex64 layout (items of 64 iterations x 32 lanes)      */
+                                   Ignored by the batched layout (items of 64 iterations x 32 lanes)        */
     int time_stages;            /* != 0: record CUDA events around each stage                        */
     int reserved[4];            /* reserved[0] != 0: purify_admm_fidelity_step runs its unfused form (separate norm and
                                    update kernels) even where the fused kernels exist; reserved[1] != 0: complex128 uses
@@ -84,9 +84,9 @@ typedef struct {
     double poly_max_abs_err;    /* ANALYTIC: max |poly - g| over the support (fit check at create)   */
     long long device_bytes;     /* device memory owned by the handle                                 */
     long long max_tile_count;   /* visibilities in the fullest tile / band                           */
-    long long M_native;         /* length of a native-order y vector (>= M: the complex64 layout pads) */
-    long long n_batches;        /* complex64 layout: batches of 32 cell-units                        */
-    int layout;                 /* 0 = tile-sorted (complex128), 1 = batched cell-stationary (complex64) */
+    long long M_native;         /* length of a native-order y vector (>= M: the batched layout pads)   */
+    long long n_batches;        /* batched layout: batches of 32 cell-units                          */
+    int layout;                 /* 0 = tile-sorted (complex128, J = 8), 1 = batched cell-stationary (complex64; complex128, J <= 6) */
     int tile_h;                 /* tile / band height in grid cells (tile = width)                   */
 } purify_info;
 

@@ -1007,7 +1007,7 @@ int purify_grid(purify_op* op, const void* y_dev, void* x_dev, void* cuda_stream
 int purify_grid_native(purify_op* op, const void* y_native_dev, void* x_dev, void* cuda_stream) {
     NEED_OP(op); NEED_PTR(x_dev, "x"); if (op->M > 0) NEED_PTR(y_native_dev, "y");
     if (op->batched && ((uintptr_t)y_native_dev & 15u))       // the kernel streams y with 16-byte-aligned bulk copies
-        return fail(PURIFY_ERR_INVALID_ARG, "y_native must be 16-byte aligned for the complex64 layout");
+        return fail(PURIFY_ERR_INVALID_ARG, "y_native must be 16-byte aligned for the batched layout");
     begin_call(op);
     return grid_impl(op, y_native_dev, x_dev, false, (cudaStream_t)cuda_stream);
 }
@@ -1172,7 +1172,7 @@ int purify_admm_fidelity_step(purify_op* op, const void* x_dev, const void* y_na
         }
         return PURIFY_OK;
     }
-    const unsigned* pm = op->batched ? op->perm : nullptr;     // padding mask (complex64 layout only)
+    const unsigned* pm = op->batched ? op->perm : nullptr;     // padding mask (batched layout only)
     // line 3: v = Phi x
     RUN(degrid_impl(op, x_dev, op->y_ws, false, st));
     // line 4: ||v + s - y||^2 (fp64 accumulation)

@@ -158,7 +158,7 @@ class PurifyOp:
 
     def permutation(self) -> torch.Tensor:
         """native -> caller index, as an int64 tensor of M_native entries on the device (copy);
-        -1 marks a padding entry of the complex64 layout."""
+        -1 marks a padding entry of the batched layout."""
         p = C.c_void_p()
         _check(self._L.purify_op_permutation(self._h, C.byref(p)), "purify_op_permutation")
         if self.M_native == 0:
