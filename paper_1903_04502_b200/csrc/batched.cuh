@@ -766,7 +766,7 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParamsT<F> p, C
 // FUSE = 1 (f1): y is v = Phi x; s and the measurements are streamed too, the gridded vector z = v - r + s_new is formed
 // slot by slot (never stored) and s_new is written to p.s_out (kernels.cuh: admm_update_kernel has the formulas).
 template <typename F, int J, int DEG, int MODE, int CH, int S, int FUSE = 0>
-__global__ void __launch_bounds__(x_warps(MODE) * 32, (MODE == 2 || sizeof(F) == 8) ? 1 : (J <= 6 ? 4 : 1))
+__global__ void __launch_bounds__(x_warps(MODE) * 32, (MODE == 2 || sizeof(F) == 8) ? 1 : (J <= 6 ? ((J == 4 ? XVG4 : XVG6) == 1 ? 4 : 3) : 1))
 grid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParamsT<F> p, const C2<F>* __restrict__ y) {
     typedef XCfg<J> Cfg;
     constexpr int NY = FUSE ? 3 : 1;
