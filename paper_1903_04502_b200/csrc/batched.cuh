@@ -11,7 +11,7 @@
 // Layout (built once at create):
 //   band   32 x 16 cells of the oversampled grid (internal DC-centred layout); one WARP works on one
 //          band at a time with a private (16+J-1) x (32+J) shared-memory box.
-//   unit   up to UNIT_CAP visibilities of ONE cell.  A cell with c visibilities gives floor(c/CAP)
+//   unit   up to UNIT_CAP (128) visibilities of ONE cell.  A cell with c visibilities gives floor(c/CAP)
 //          full units and one remainder unit.
 //   batch  32 consecutive units of the band's unit sequence, one per lane, processed in lockstep for
 //          n_iter = (count of the batch's first unit) iterations.  The sequence is: the full units in
@@ -37,7 +37,10 @@
 namespace pk {
 
 constexpr int XBW = 32, XBH = 16, XCELLS = XBW * XBH;   // band geometry
-constexpr int UNIT_CAP = 64;                            // visibilities per unit
+#ifndef PURIFY_UNIT_CAP
+#define PURIFY_UNIT_CAP 128
+#endif
+constexpr int UNIT_CAP = PURIFY_UNIT_CAP;                            // visibilities per unit
 #ifndef PURIFY_ITEM_ITERS
 #define PURIFY_ITEM_ITERS 64
 #endif

@@ -280,8 +280,8 @@ def test_hot_cells_and_layer_straddling_batches():
     rng = synth.rng_for(4242, synth.STREAM_UV)
     n, J = 64, 6
     K = 2 * n
-    hot = rng.integers(-20, 20, size=(7, 2)).astype(np.float64)
-    counts = [700, 333, 129, 128, 65, 64, 63]
+    counts = [700, 333, 257, 256, 129, 128, 127, 65, 64, 63]          # around multiples of the unit capacity
+    hot = rng.integers(-20, 20, size=(len(counts), 2)).astype(np.float64)
     parts = [h + rng.uniform(0.0, 1.0, size=(c, 2)) for h, c in zip(hot, counts)]
     parts.append(rng.uniform(-K / 2, K / 2, size=(3000, 2)))
     uv = np.concatenate(parts)
