@@ -402,9 +402,12 @@ __device__ __forceinline__ void x_weights(C2<F> uv, C2<F> cellf, int cx, int cy,
             const F dx = sub_rn(uv.x, (F)ox), dy = sub_rn(uv.y, (F)oy);
             const int ix = (int)floor_r(add_rn(mul_rn(fabs(dx), p.table_R), (F)0.5));
             const int iy = (int)floor_r(add_rn(mul_rn(fabs(dy), p.table_R), (F)0.5));
-            // MODE 1: table in global memory (read through L1); MODE 2: the CTA's copy in shared memory
-            g[j].x = ix < p.table_len ? (MODE == 2 ? tab[ix] : __ldg(tab + ix)) : (F)0;
-            g[j].y = iy < p.table_len ? (MODE == 2 ? tab[iy] : __ldg(tab + iy)) : (F)0;
+            // MODE 1: table in global memory (read through L1); MODE 2: the CTA's copy in shared memory.  A real slot's
+            // (u, v) lies in its unit's cell, so |d| <= J/2 and the index is at most R J/2; the clamp only serves the
+            // slots of idle lanes (no unit, w = 0): the last table entry is g beyond the support, 0.
+            const int jx = min(ix, p.table_len - 1), jy = min(iy, p.table_len - 1);
+            g[j].x = MODE == 2 ? tab[jx] : __ldg(tab + jx);
+            g[j].y = MODE == 2 ? tab[jy] : __ldg(tab + jy);
         }
     }
 }
