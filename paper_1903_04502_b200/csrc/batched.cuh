@@ -186,12 +186,21 @@ band_build_kernel(const unsigned* __restrict__ keys, const unsigned* __restrict_
     __syncthreads();
     if (myfull) { atomicAdd(&s_F, myfull); atomicMax(&s_maxfull, myfull); }
     if (myrem) atomicAdd(&s_Rn, 1u);
-    // rank of the remainder unit: descending count, ties by cell (zeros sort last)
-    unsigned rank = 0;
-    for (int q = 0; q < XCELLS; ++q) {
-        const unsigned e = s_rem[q];
-        rank += (e > myrem || (e == myrem && q < t)) ? 1u : 0u;
+    // rank of the remainder unit: descending count (zeros sort last).  Units of EQUAL count are ordered so that 32
+    // consecutive ones spread over the 16 shared-memory bank classes: by their index among the cells of the same count
+    // and class first, then by class, then by cell.  (Which equal-count unit lands in which batch costs no padding.)
+    const unsigned mycls = (((unsigned)t >> 5) * (unsigned)boxw + ((unsigned)t & 31u)) & 15u;
+    unsigned ric = 0;
+    for (int q = 0; q < t; ++q) {
+        const unsigned cq = (((unsigned)q >> 5) * (unsigned)boxw + ((unsigned)q & 31u)) & 15u;
+        ric += (s_rem[q] == myrem && cq == mycls) ? 1u : 0u;
     }
+    const unsigned mykey = ((unsigned)(UNIT_CAP - myrem) << 19) | (ric << 13) | (mycls << 9) | (unsigned)t;
+    s_scan[t] = mykey;                                   // (s_scan is free until the batch scan below)
+    __syncthreads();
+    unsigned rank = 0;
+    for (int q = 0; q < XCELLS; ++q) rank += s_scan[q] < mykey ? 1u : 0u;
+    __syncthreads();
     s_remsorted[rank] = myrem;
     __syncthreads();
     const unsigned F = s_F, Rn = s_Rn, maxfull = s_maxfull;
