@@ -146,7 +146,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    from paper_1903_04502_b200 import synth
+    from inputs import synth
     cfg = synth.CONFIGS[args.config]
     M = args.M or cfg.M
     ms = min(args.cpu_sample, M)
@@ -210,7 +210,8 @@ def run_ours(args):
     import torch
     import torch.distributed as dist
 
-    from paper_1903_04502_b200 import ANALYTIC, C64, C128, TABLE, PurifyOp, synth
+    from inputs import synth
+    from paper_1903_04502_b200 import ANALYTIC, C64, C128, TABLE, PurifyOp
     from paper_1903_04502_b200 import dist as pdist
 
     rank, local_rank, world = pdist.world()

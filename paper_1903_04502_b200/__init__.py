@@ -2,7 +2,7 @@
 
     from paper_1903_04502_b200 import PurifyOp
 
-`synth` (seeded input generators) is importable without CUDA; `op` needs the built C-ABI library
-(`python -m paper_1903_04502_b200.build`) and fails loudly without it - there is no CPU fallback.
+`op` needs the built C-ABI library (`python -m paper_1903_04502_b200.build`) and fails loudly without it -
+there is no CPU fallback.  The seeded input generators live outside the package, in `inputs/`.
 """
 from .op import ANALYTIC, C64, C128, TABLE, PurifyError, PurifyOp, load_library  # noqa: F401

@@ -37,28 +37,13 @@
 namespace pk {
 
 constexpr int XBW = 32, XBH = 16, XCELLS = XBW * XBH;   // band geometry
-#ifndef PURIFY_UNIT_CAP
-#define PURIFY_UNIT_CAP 128
-#endif
-constexpr int UNIT_CAP = PURIFY_UNIT_CAP;                            // visibilities per unit
-#ifndef PURIFY_ITEM_ITERS
-#define PURIFY_ITEM_ITERS 64
-#endif
-constexpr int ITEM_ITERS = PURIFY_ITEM_ITERS;                         // iterations per item
+constexpr int UNIT_CAP = 128;                           // visibilities per unit
+constexpr int ITEM_ITERS = 64;                          // iterations per item
 constexpr unsigned PERM_PAD = 0xFFFFFFFFu;
-constexpr int REC_FLOATS = 96, REC_BYTES = 384;
-#ifndef PURIFY_XVD
-#define PURIFY_XVD 2
-#endif
-#ifndef PURIFY_XVG
-#define PURIFY_XVG 1
-#endif
-#ifndef PURIFY_XVG4
-#define PURIFY_XVG4 1
-#endif
+constexpr int REC_FLOATS = 96, REC_BYTES = 384;         // per-iteration record: uv[32] | w[32]
 // visibilities per inner-loop trip (statement-interleaved dependency graphs): degridding gains from 2 (0.73 ->
 // 0.69 ms at config 4, 160 registers, 3 CTAs / SM); gridding loses (its flush phases want the 4th CTA)
-constexpr int XVD = PURIFY_XVD, XVG6 = PURIFY_XVG, XVG4 = PURIFY_XVG4;         // per-iteration record: uv[32] | w[32]
+constexpr int XVD = 2, XVG6 = 1, XVG4 = 1;
 
 template <int J> struct XCfg {
     static constexpr int XOFF = (J / 2 - 1) & 1;        // makes the box's first column even (TMA: 16-byte aligned)
@@ -83,7 +68,8 @@ template <typename F> struct XParamsT {
     int K, Kh, kmask;
     const XItem* items;
     int n_items;
-    unsigned* counter;            // dynamic item queue (reset before every launch)
+    unsigned* counter;            // [0] dynamic item queue, [1] warps finished: the last warp to leave zeroes both
+    int n_warps;                  // persistent warps of this launch
     const uint2* bhdr;            // per batch: x = first iteration, y = n_iter | flags << 16 (bit 0: a cell may occur twice)
     const unsigned* blane;        // per batch 32 lane words: cell (ly << 5 | lx) | count << 16
     const F* rec;             // per-iteration records (REC_FLOATS floats each)
@@ -392,7 +378,7 @@ __device__ __forceinline__ void x_weights(C2<F> uv, C2<F> cellf, int cx, int cy,
                                           C2<F> (&g)[J]) {
     if (MODE == 0) {
         constexpr int NE = DEG / 2 + 1, NO = (DEG + 1) / 2;
-        const C2<F> t = add2(add2(uv, mk2<F>(-cellf.x, -cellf.y)), mk2<F>((F)-0.5, (F)-0.5));
+        const C2<F> t = add2(uv, mk2<F>(-cellf.x - (F)0.5, -cellf.y - (F)0.5));     // cell + 1/2 is exact; so is u - cell
         const C2<F> t2 = mul2(t, t), nt = mk2<F>(-t.x, -t.y);
 #pragma unroll
         for (int j = 0; j < J / 2; ++j) {
@@ -431,7 +417,7 @@ __device__ __forceinline__ void x_weights_v(const C2<F> (&uv)[V], C2<F> cellf, i
         C2<F> t[V], t2[V], nt[V];
 #pragma unroll
         for (int v = 0; v < V; ++v) {
-            t[v] = add2(add2(uv[v], mk2<F>(-cellf.x, -cellf.y)), mk2<F>((F)-0.5, (F)-0.5));
+            t[v] = add2(uv[v], mk2<F>(-cellf.x - (F)0.5, -cellf.y - (F)0.5));       // cell + 1/2 is exact; so is u - cell
             t2[v] = mul2(t[v], t[v]);
             nt[v] = mk2<F>(-t[v].x, -t[v].y);
         }
@@ -514,6 +500,18 @@ __device__ __forceinline__ unsigned x_next_item(unsigned* counter, int lane) {
     unsigned it = 0;
     if (lane == 0) it = atomicAdd(counter, 1u);
     return __shfl_sync(0xffffffffu, it, 0);
+}
+// Kernel tail: the last persistent warp to leave resets the queue, so that launches need no memset in between
+// (every warp's pops precede its own arrival here; launches of one handle are ordered by the stream).
+__device__ __forceinline__ void x_queue_finish(unsigned* counter, int n_warps, int lane) {
+    if (lane == 0) {
+        __threadfence();
+        if (atomicAdd(counter + 1, 1u) == (unsigned)n_warps - 1u) {
+            counter[0] = 0;
+            counter[1] = 0;
+            __threadfence();
+        }
+    }
 }
 
 // a0.6: longest items first (LPT order of the dynamic queue: the tail of a launch then consists of short items).
@@ -728,7 +726,7 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParamsT<F> p, C
                             if (i + k + v < cnt) {                          // a real slot: d = v + s - y
                                 const C2<F> sv = sp[v * 32], yv = sp[CH * 32 + v * 32];
                                 const F dx = (o[v].x + sv.x) - yv.x, dy = (o[v].y + sv.y) - yv.y;
-                                nacc += (double)(dx * dx + dy * dy);
+                                nacc += (double)dx * (double)dx + (double)dy * (double)dy;
                             }
                         sp += XVK * 32;
                     }
@@ -745,7 +743,7 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParamsT<F> p, C
                         if (i + k < cnt) {
                             const C2<F> sv = sp[0], yv = sp[CH * 32];
                             const F dx = (o1[0].x + sv.x) - yv.x, dy = (o1[0].y + sv.y) - yv.y;
-                            nacc += (double)(dx * dx + dy * dy);
+                            nacc += (double)dx * (double)dx + (double)dy * (double)dy;
                         }
                         sp += 32;
                     }
@@ -767,6 +765,7 @@ degrid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParamsT<F> p, C
         for (int o = 16; o > 0; o >>= 1) nacc += __shfl_down_sync(0xffffffffu, nacc, o);
         if (lane == 0) atomicAdd(p.norm2, nacc);
     }
+    x_queue_finish(p.counter, p.n_warps, lane);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -937,17 +936,17 @@ grid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParamsT<F> p, con
                 // instructions in issue order; the volatile asm keeps the compiler from reordering them.
                 // (A __syncwarp() per step is semantically the same and costs a BRA.DIV + NOP per tap.)
                 __syncwarp();
-                if (cnt > 0) {
+                {
                     const uint32_t da = smem_u32(dst);
 #pragma unroll
                     for (int a = 0; a < J; ++a)
 #pragma unroll
                         for (int c = 0; c < J; ++c) {
                             const uint32_t ad = da + (uint32_t)(a * BOXW + c) * (uint32_t)sizeof(C2<F>);
-                            sts_v2(ad, add2(lds_v2<F>(ad), A[a][c]));
+                            if (cnt > 0) sts_v2(ad, add2(lds_v2<F>(ad), A[a][c]));
+                            __syncwarp();
                         }
                 }
-                __syncwarp();
             } else {
                 if (cnt > 0) {
 #pragma unroll
@@ -985,6 +984,7 @@ grid_x_kernel(const __grid_constant__ CUtensorMap tmap, const XParamsT<F> p, con
         __syncwarp();
     }
     if (lane == 0) bulk_wait_group_read0();             // shared memory must outlive the last reduction's reads
+    x_queue_finish(p.counter, p.n_warps, lane);
 }
 
 }  // namespace pk

@@ -14,6 +14,7 @@
 #include <cstdint>
 #include <cstdio>
 #include <cstring>
+#include <map>
 #include <new>
 #include <vector>
 
@@ -109,7 +110,7 @@ struct purify_op {
     pk::XItem* x_items = nullptr;
     unsigned* x_counter = nullptr;
     CUtensorMap tmap_x;
-    int x_ctas_degrid = 0, x_ctas_grid = 0;
+    std::map<const void*, int> x_ctas;   // persistent grid size per kernel instantiation (occupancy query done once)
 };
 
 namespace {
@@ -213,8 +214,12 @@ template <typename F> pk::XParamsT<F> make_xparams(const purify_op* op) {
     return p;
 }
 
-// persistent grid: as many CTAs as fit on the device at once (capped by the number of items)
-template <typename Kern> int x_grid_size(Kern kern, int threads, size_t smem, int n_items, int warps, int* out) {
+// persistent grid: as many CTAs as fit on the device at once (capped by the number of items).  The occupancy query
+// and the shared-memory attribute are done once per handle and kernel instantiation, not per launch.
+template <typename Kern> int x_grid_size(purify_op* op, Kern kern, int threads, size_t smem, int warps, int* out) {
+    const void* key = (const void*)kern;
+    auto hit = op->x_ctas.find(key);
+    if (hit != op->x_ctas.end()) { *out = hit->second; return PURIFY_OK; }
     int dev = 0, sms = 0, per_sm = 0;
     CK(cudaGetDevice(&dev));
     CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
@@ -222,22 +227,16 @@ template <typename Kern> int x_grid_size(Kern kern, int threads, size_t smem, in
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem));
     if (per_sm < 1) per_sm = 1;
     int g = sms * per_sm;
-    const int need = (n_items + warps - 1) / warps;
+    const int need = (op->n_items + warps - 1) / warps;
     if (g > need) g = need;
     if (g < 1) g = 1;
+    op->x_ctas[key] = g;
     *out = g;
     return PURIFY_OK;
 }
 
-// ring geometry of the complex64 kernels: CH iterations per chunk, S stages (batched.cuh "ring")
-// ring geometry (chunk iterations, stages) of the two complex64 kernels; -D overrides are for tuning builds
-#ifndef PURIFY_X_CHD
-#define PURIFY_X_CHD 16
-#define PURIFY_X_SD 2
-#define PURIFY_X_CHG 6
-#define PURIFY_X_SG 2
-#endif
-constexpr int X_CH_DEGRID = PURIFY_X_CHD, X_S_DEGRID = PURIFY_X_SD, X_CH_GRID = PURIFY_X_CHG, X_S_GRID = PURIFY_X_SG;
+// ring geometry (iterations per chunk, stages) of the two complex64 kernels (batched.cuh "ring")
+constexpr int X_CH_DEGRID = 16, X_S_DEGRID = 2, X_CH_GRID = 6, X_S_GRID = 2;
 // TABLE mode.  A table of up to 64 KB (R J/2 + 2 floats; 32 KB at R = 4096, J = 4) is copied into shared memory by
 // every CTA (MODE 2, 8 warps per CTA): 32 lanes looking up unrelated entries cost ~3.5 shared-memory wavefronts per
 // lookup, against many more L1 tag look-ups when the table sits in global memory.  Larger tables (the paper's
@@ -256,10 +255,10 @@ int launch_degrid_x_m(purify_op* op, void* y, size_t extra_smem, cudaStream_t st
     const size_t smem = pk::XSmem<F, J, CH, S, FUSE ? 2 : 0, NW>::TOTAL + extra_smem;
     pk::XParamsT<F> p = make_xparams<F>(op);
     if (aa) { p.s_in = (const F2*)aa->s; p.yobs = (const F2*)aa->y_obs; p.s_out = (F2*)aa->s; p.eps = aa->eps; p.varrho = aa->varrho; }
-    CK(cudaMemsetAsync(op->x_counter, 0, sizeof(unsigned), st));
     int g = 0, rc;
     auto kern = pk::degrid_x_kernel<F, J, DEG, MODE, CH, S, FUSE>;
-    if ((rc = x_grid_size(kern, NW * 32, smem, op->n_items, NW, &g))) return rc;
+    if ((rc = x_grid_size(op, kern, NW * 32, smem, NW, &g))) return rc;
+    p.n_warps = g * NW;
     kern<<<g, NW * 32, smem, st>>>(op->tmap_x, p, (F2*)y);
     op->launches++;
     CK(cudaGetLastError());
@@ -273,10 +272,10 @@ int launch_grid_x_m(purify_op* op, const void* y, size_t extra_smem, cudaStream_
     const size_t smem = pk::XSmem<F, J, CH, S, FUSE ? 3 : 1, NW>::TOTAL + extra_smem;
     pk::XParamsT<F> p = make_xparams<F>(op);
     if (aa) { p.s_in = (const F2*)aa->s; p.yobs = (const F2*)aa->y_obs; p.s_out = (F2*)aa->s; p.eps = aa->eps; p.varrho = aa->varrho; }
-    CK(cudaMemsetAsync(op->x_counter, 0, sizeof(unsigned), st));
     int g = 0, rc;
     auto kern = pk::grid_x_kernel<F, J, DEG, MODE, CH, S, FUSE>;
-    if ((rc = x_grid_size(kern, NW * 32, smem, op->n_items, NW, &g))) return rc;
+    if ((rc = x_grid_size(op, kern, NW * 32, smem, NW, &g))) return rc;
+    p.n_warps = g * NW;
     kern<<<g, NW * 32, smem, st>>>(op->tmap_x, p, (const F2*)y);
     op->launches++;
     CK(cudaGetLastError());
@@ -682,7 +681,8 @@ int build_bins_x(purify_op* op, const void* uv_dev, const void* w_dev, cudaStrea
     if ((rc = dev_alloc(op, (void**)&op->x_bhdr, sizeof(uint2) * NBz))) { cleanup(); return rc; }
     if ((rc = dev_alloc(op, (void**)&op->x_blane, sizeof(unsigned) * 32 * NBz))) { cleanup(); return rc; }
     if ((rc = dev_alloc(op, (void**)&op->x_items, sizeof(pk::XItem) * (size_t)(op->n_items > 0 ? op->n_items : 1)))) { cleanup(); return rc; }
-    if ((rc = dev_alloc(op, (void**)&op->x_counter, sizeof(unsigned)))) { cleanup(); return rc; }
+    if ((rc = dev_alloc(op, (void**)&op->x_counter, 2 * sizeof(unsigned)))) { cleanup(); return rc; }
+    CKC(cudaMemsetAsync(op->x_counter, 0, 2 * sizeof(unsigned), st));     // the kernels leave the queue at 0 (batched.cuh x_queue_finish)
     CKC(cudaMalloc(&lsrc, sizeof(unsigned) * 32 * NBz));
     if (op->n_batches > 0) {
         pk::band_build_kernel<2><<<n_bands, pk::XCELLS, 0, st>>>(keys2, band_start, nbx, pk::XBW + op->J, nullptr, o_nb, o_it, o_items,

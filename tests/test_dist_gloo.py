@@ -12,7 +12,7 @@ import torch.multiprocessing as mp
 
 import oracle
 from paper_1903_04502_b200 import dist as pdist
-from paper_1903_04502_b200 import synth
+from inputs import synth
 
 
 def _free_port():

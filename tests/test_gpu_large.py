@@ -12,7 +12,7 @@ import pytest
 import torch
 
 import oracle
-from paper_1903_04502_b200 import synth
+from inputs import synth
 
 pytestmark = [pytest.mark.gpu, pytest.mark.slow]
 

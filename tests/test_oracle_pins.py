@@ -10,7 +10,7 @@ import scipy.integrate
 import scipy.special
 
 import oracle
-from paper_1903_04502_b200 import synth
+from inputs import synth
 
 GOLD = {}
 with open(os.path.join(os.path.dirname(__file__), "golden", "constants.txt")) as fh:

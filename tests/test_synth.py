@@ -1,7 +1,7 @@
 """Seeded generators: determinism, ranges, shapes (no method arithmetic in synth).  -m "not gpu" """
 import numpy as np
 
-from paper_1903_04502_b200 import synth
+from inputs import synth
 
 
 def test_image_recipe():
