@@ -30,7 +30,9 @@
  *           result is in host memory) and purify_stage_times_ms synchronise.
  *   errors  every function returns a purify_status (0 = OK, < 0 = error); nothing throws, aborts or
  *           prints.  purify_last_error() gives a thread-local detail string for the last failure.
- *   thread  a handle is not re-entrant (one workspace); distinct handles are independent.
+ *   thread  a handle is NOT re-entrant: it owns one grid workspace, one work queue and one set of lazily allocated
+ *           vectors, so two calls on the same handle must not overlap - neither from two host threads nor on two
+ *           streams (calls on ONE stream are ordered and fine).  Distinct handles are independent.
  *   determinism  degrid is bit-reproducible.  grid/normal flush partial tiles with floating-point
  *           atomics, so the last bits of the gridded image may vary from call to call.
  */
@@ -65,11 +67,14 @@ typedef struct {
                                    T[i] = g(i/R), i = 0..R*J/2+1, lookup T[floor(|d| R + 1/2)].      */
     int chunk;                  /* complex128 (tile-sorted layout): visibilities per work item (CTA); default 4096.
                                    Ignored by the batched layout (items of 64 iterations x 32 lanes)        */
-    int time_stages;            /* != 0: record CUDA events around each stage                        */
-    int reserved[4];            /* reserved[0] != 0: purify_admm_fidelity_step runs its unfused form (separate norm and
-                                   update kernels) even where the fused kernels exist; reserved[1] != 0: complex128 uses
-                                   the tile-sorted kernels for every J (default: batched layout for J <= 6, tile-sorted
-                                   for J = 8); others must be 0                                                      */
+    int time_stages;            /* != 0: record CUDA events around each stage (also switchable later:
+                                   purify_op_set_time_stages); while it is on, purify_normal is not replayed
+                                   from its CUDA graph                                                        */
+    int admm_unfused;           /* != 0: purify_admm_fidelity_step runs its unfused form (separate norm and update
+                                   kernels) even where the fused kernels exist                                */
+    int force_tile_sorted;      /* != 0: complex128 uses the tile-sorted kernels for every J (default: batched
+                                   layout for J <= 6, tile-sorted for J = 8)                                   */
+    int reserved[2];            /* must be 0                                                                   */
 } purify_opts;
 
 /* Facts about a handle (for tests, benches and roofline arithmetic). */
@@ -140,6 +145,22 @@ int purify_degrid_host(purify_op *op, const void *x_host, void *y_host, void *cu
 int purify_grid_host(purify_op *op, const void *y_host, void *x_host, void *cuda_stream);
 int purify_normal_host(purify_op *op, const void *x_in_host, void *x_out_host, void *cuda_stream);
 
+/* f3: the distributed-image operator - "each node has a replica of the image and its own section of
+ * the visibilities": Phi_j needs no exchange (Eq. 37), x' = sum_j Phi_j^dagger y_j is an all-reduce
+ * of the n x n image (Eq. 38; Algorithm 2 "AllSumAll").  The exchange is the CALLER's: these two
+ * calls run Phi_j^dagger (resp. Phi_j^dagger Phi_j) and hand the image to `allreduce` in `bands` horizontal bands
+ * (rows [n k / bands, n (k+1) / bands)) as each leaves the crop kernel, so that band k is reduced while band k + 1 is
+ * cropped; when the call returns, work enqueued on cuda_stream afterwards sees the reduced image.
+ *   allreduce(user, band_dev, count_reals, is_double, comm_stream) must ENQUEUE an in-place sum over the ranks of the
+ *   count_reals floats (is_double = 0) or doubles at band_dev onto comm_stream (a stream owned by the handle, already
+ *   ordered after the band's crop) and return 0; e.g. ncclAllReduce(band_dev, band_dev, count_reals, ncclFloat,
+ *   ncclSum, comm, comm_stream).  allreduce = NULL: a single process, no exchange.  y in native order (M_native). */
+typedef int (*purify_allreduce_fn)(void *user, void *band_dev, long long count_reals, int is_double, void *comm_stream);
+int purify_grid_dist(purify_op *op, const void *y_native_dev, void *x_dev, int bands,
+                     purify_allreduce_fn allreduce, void *user, void *cuda_stream);
+int purify_normal_dist(purify_op *op, const void *x_in_dev, void *x_out_dev, int bands,
+                       purify_allreduce_fn allreduce, void *user, void *cuda_stream);
+
 /* f2: largest eigenvalue of Phi^dagger Phi = ||Phi||^2 by the power method ("We can normalize the
  * operator with the operator norm, by using the power method to estimate the largest eigenvalue").
  * x_1 = x0 / ||x0||; z_k = Phi^dagger Phi x_k; lambda_k = ||z_k||_2; x_{k+1} = z_k / lambda_k; stops after max_iter
@@ -169,10 +190,20 @@ int purify_admm_fidelity_step(purify_op *op, const void *x_dev, const void *y_na
 int purify_stage_fourier_grid(purify_op *op, const void *x_dev, void *B_dev /* K*K complex */, void *cuda_stream);
 int purify_stage_gridded(purify_op *op, const void *y_dev /* caller order */, void *B_dev, void *cuda_stream);
 
-/* Milliseconds per stage of the last call (needs opts.time_stages); synchronises. */
+/* Milliseconds per stage of the last call (needs stage timing switched on); synchronises. */
 int purify_stage_times_ms(const purify_op *op, float out[PURIFY_STAGE_COUNT]);
+/* Switch the per-stage CUDA events on (enable != 0) or off for the calls that follow. */
+int purify_op_set_time_stages(purify_op *op, int enable);
 /* Number of kernels of this library (cuFFT launches not counted) enqueued by the last call. */
 int purify_last_launch_count(const purify_op *op);
+
+/* Measurement aid: issue rate of the packed fp32 instruction forms the hot kernels consist of, on the
+ * current device.  form 0: 2 x FFMA (3 registers); 1: FFMA2 broadcast scalar x pair + pair (degridding row pass);
+ * 2: FFMA2 pair x pair + pair; 3: FFMA2 pair x pair + constant (Horner step); 4: FFMA2 varying scalar x shared pair +
+ * pair (gridding).  warps_per_sm in {4, 8, ..., 32}.  *cycles_per_instr_out (HOST): SM cycles per warp instruction per
+ * SM sub-partition, from clock64() inside the kernel; *sm_ghz_out (HOST, may be NULL): cycles / event time.
+ * Allocates and frees its own scratch, uses the legacy default stream and synchronises. */
+int purify_ubench_fma(int form, int warps_per_sm, double *cycles_per_instr_out, double *sm_ghz_out);
 
 const char *purify_strerror(int status);
 const char *purify_last_error(void);

@@ -41,6 +41,7 @@ def lib():
         L.oracle_table.argtypes = [C.c_int, C.c_int, _dp]
         L.oracle_kernel_weight.restype = C.c_double
         L.oracle_kernel_weight.argtypes = [C.c_double, C.c_long, C.c_int, C.c_int, C.c_int, C.c_int]
+        L.oracle_table_index.argtypes = [C.c_long, _dp, C.POINTER(C.c_long), C.c_int, C.c_int, C.POINTER(C.c_long)]
         L.oracle_fft2.argtypes = [_dp, C.c_int, C.c_int]
         L.oracle_dft2_direct.argtypes = [_dp, _dp, C.c_int, C.c_int]
         L.oracle_pad.argtypes = [C.c_int, C.c_int, _dp, _dp]
@@ -118,6 +119,17 @@ def table(J: int, R: int) -> np.ndarray:
 
 def kernel_weight(u: float, c: int, J: int, mode="analytic", R: int = 4096, idx_prec: int = 64) -> float:
     return float(lib().oracle_kernel_weight(float(u), int(c), int(J), _mode(mode), int(R), int(idx_prec)))
+
+
+def table_index(u, c, R: int = 4096, idx_prec: int = 64) -> np.ndarray:
+    """R11: floor(|u - c| R + 1/2) for arrays of coordinates u and taps c, decided in fp32 (idx_prec 32) or fp64."""
+    u = np.ascontiguousarray(u, dtype=np.float64)
+    c = np.ascontiguousarray(c, dtype=np.int64)
+    assert u.shape == c.shape and u.ndim == 1
+    out = np.empty(len(u), dtype=np.int64)
+    lp = C.POINTER(C.c_long)
+    lib().oracle_table_index(len(u), _p(u), c.ctypes.data_as(lp), int(R), int(idx_prec), out.ctypes.data_as(lp))
+    return out
 
 
 def fft2(a: np.ndarray, sign: int = -1) -> np.ndarray:

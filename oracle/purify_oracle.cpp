@@ -15,7 +15,9 @@
 // sum_c g(delta-c) closed form, g-hat vs numerical quadrature, FFT vs direct DFT and
 // numpy, Phi vs brute-force NUDFT (Eq. 1), adjoint identity, centred / off-centre point
 // sources, single-visibility adjoint, periodic wrap, table accuracy.
-// Parity unpinned by the paper: the tie-break at integer u (R7) - convention only.
+// The tap set of W G at integer / half-integer (u, v) (R7) is pinned on a one-hot Fourier grid and through the adjoint
+// identity at such coordinates; the fp32 branch of the table index (R11) against exact integer arithmetic.
+// Parity unpinned by the paper: WHICH of the two equally valid tie-breaks at integer u is taken (R7) - convention only.
 //
 // Conventions: image x[py*n+px] complex interleaved (re,im), px fastest, px<->u, py<->v;
 // centred pixel coordinate p^ = p - n/2; grid side K = 2n; (u,v) in grid cells, period K.
@@ -94,6 +96,21 @@ static void build_table(int J, int R, std::vector<double>& T) {
 // evaluated in double; idx_prec 32: in float (the CUDA C64 path's precision - task
 // rule 3: "where floating point decides an integer, both sides take that decision in
 // the same precision").  u arrives already rounded to the storage precision.
+// R11: index of the nearest table sample for the distance |u - c|: floor(|d| R + 1/2), each step ONE IEEE operation
+// in the storage precision of the problem (idx_prec 32: float, 64: double).
+static long table_index(double u, long c, int R, int idx_prec) {
+    if (idx_prec == 32) {
+        volatile float df = (float)u - (float)c;          // one IEEE fp32 subtraction
+        volatile float a = std::fabs(df) * (float)R;      // one fp32 multiply
+        volatile float b = a + 0.5f;                      // one fp32 add
+        return (long)std::floor((double)b);
+    }
+    volatile double d = u - (double)c;
+    volatile double a = std::fabs(d) * (double)R;
+    volatile double b = a + 0.5;
+    return (long)std::floor(b);
+}
+
 struct KernelEval {
     int J, mode, R, idx_prec;
     std::vector<double> T;
@@ -102,18 +119,7 @@ struct KernelEval {
     }
     double operator()(double u, long c) const {
         if (mode == 0) return kb_g(u - (double)c, J);
-        long idx;
-        if (idx_prec == 32) {
-            volatile float df = (float)u - (float)c;          // one IEEE fp32 subtraction
-            volatile float a = std::fabs(df) * (float)R;      // one fp32 multiply
-            volatile float b = a + 0.5f;                      // one fp32 add
-            idx = (long)std::floor((double)b);
-        } else {
-            volatile double d = u - (double)c;
-            volatile double a = std::fabs(d) * (double)R;
-            volatile double b = a + 0.5;
-            idx = (long)std::floor(b);
-        }
+        const long idx = table_index(u, c, R, idx_prec);
         if (idx >= (long)T.size()) return 0.0;
         return T[idx];
     }
@@ -321,6 +327,11 @@ void oracle_table(int J, int R, double* T_out) {
 double oracle_kernel_weight(double u, long c, int J, int mode, int R, int idx_prec) {
     KernelEval ker(J, mode, R, idx_prec);
     return ker(u, c);
+}
+
+// the table index rule on its own, for n (u, c) pairs (pin of the idx_prec = 32 branch)
+void oracle_table_index(long n, const double* u, const long* c, int R, int idx_prec, long* out) {
+    for (long i = 0; i < n; ++i) out[i] = table_index(u[i], c[i], R, idx_prec);
 }
 
 // in-place unnormalised 2-D DFT of a K x K complex array, sign = -1 forward, +1 adjoint

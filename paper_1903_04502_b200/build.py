@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpurify_op.so")
 SOURCES = ["purify_op.cu"]
-DEPS = ["purify_op.cu", "kernels.cuh", "degrid.cuh", "grid.cuh", "batched.cuh", "kb_host.hpp",
+DEPS = ["purify_op.cu", "kernels.cuh", "degrid.cuh", "grid.cuh", "batched.cuh", "kb_host.hpp", "ubench.cuh",
         os.path.join("..", "..", "include", "purify_op.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared"]

@@ -174,15 +174,16 @@ __global__ void __launch_bounds__(256) pad_kernel(const typename Cplx<R>::type* 
     }
 }
 
-// a6: Z^dagger S^dagger fused: x'[py,px] = sign s[py] s[px] b'[p^y mod K, p^x mod K].
+// a6: Z^dagger S^dagger fused: x'[py,px] = sign s[py] s[px] b'[p^y mod K, p^x mod K], image rows [row0, row1)
+// (the whole image, or one band of it when the bands are handed to an all-reduce one by one, f3).
 template <typename R>
 __global__ void __launch_bounds__(256) crop_kernel(const typename Cplx<R>::type* __restrict__ b,
                                                    const R* __restrict__ s, typename Cplx<R>::type* __restrict__ x,
-                                                   int n, int K) {
+                                                   int n, int K, int row0, int row1) {
     typedef typename Cplx<R>::type C;
     const int nh = n / 2;
-    const long long total = (long long)n * n;
-    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total;
+    const long long first = (long long)row0 * n, total = (long long)row1 * n;
+    for (long long i = first + blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total;
          i += (long long)gridDim.x * blockDim.x) {
         const int py = (int)(i / n), px = (int)(i % n);
         const int jy = py >= nh ? py - nh : py + K - nh;

@@ -23,6 +23,7 @@
 #include "grid.cuh"
 #include "kb_host.hpp"
 #include "kernels.cuh"
+#include "ubench.cuh"
 
 namespace {
 
@@ -86,11 +87,12 @@ struct purify_op {
     void* corr = nullptr;     // s[n]
     void* table = nullptr;
     int table_len = 0;
-    void* y_ws = nullptr;     // M complex (purify_normal / host paths), lazily allocated
+    void* y_ws = nullptr;     // M_native complex (purify_normal / host paths), lazily allocated
     void* x_ws = nullptr;     // n*n complex staging for host paths
-    void* y_ws2 = nullptr;    // caller-order staging for host paths
+    void* y_ws2 = nullptr;    // caller-order staging for host paths / z of the unfused ADMM step
+    size_t y_ws_bytes = 0, x_ws_bytes = 0, y_ws2_bytes = 0, scal_ws_bytes = 0;
     double* scal_ws = nullptr; // one fp64 scalar (norms)
-    bool admm_unfused = false; // opts.reserved[0] != 0: purify_admm_fidelity_step uses separate norm / update kernels
+    bool admm_unfused = false; // opts.admm_unfused: purify_admm_fidelity_step uses separate norm / update kernels
     cufftHandle plan = 0;
     bool plan_ok = false;
     CUtensorMap tmap;
@@ -111,6 +113,17 @@ struct purify_op {
     unsigned* x_counter = nullptr;
     CUtensorMap tmap_x;
     std::map<const void*, int> x_ctas;   // persistent grid size per kernel instantiation (occupancy query done once)
+    // purify_normal replayed from a CUDA graph (captured on an internal stream, launched on the caller's)
+    cudaStream_t cap_stream = nullptr;
+    cudaGraphExec_t normal_exec = nullptr;
+    const void* normal_in = nullptr;
+    void* normal_out = nullptr;
+    int normal_launches = 0;
+    bool graph_stale = false, graph_failed = false, normal_warm = false;
+    // f3: side stream on which the caller's all-reduce of the image bands is enqueued, and the events that chain it
+    cudaStream_t comm_stream = nullptr;
+    std::vector<cudaEvent_t> band_ev;
+    cudaEvent_t comm_done = nullptr;
 };
 
 namespace {
@@ -396,16 +409,20 @@ int launch_pad(purify_op* op, const void* x, cudaStream_t st) {
     return PURIFY_OK;
 }
 
-int launch_crop(purify_op* op, void* x, cudaStream_t st) {
-    StageTimer t(op, PURIFY_STAGE_CROP, st);
-    const long long tot = (long long)op->n * op->n;
-    if (op->dtype == PURIFY_C64)
-        pk::crop_kernel<float><<<grid_for(tot, 256, 148 * 32), 256, 0, st>>>((const float2*)op->grid, (const float*)op->corr,
-                                                                             (float2*)x, op->n, op->K);
-    else
-        pk::crop_kernel<double><<<grid_for(tot, 256, 148 * 32), 256, 0, st>>>((const double2*)op->grid, (const double*)op->corr,
-                                                                              (double2*)x, op->n, op->K);
-    op->launches++;
+int launch_crop(purify_op* op, void* x, cudaStream_t st, int row0 = 0, int row1 = -1, bool timed = true) {
+    if (row1 < 0) row1 = op->n;
+    if (timed && op->time_stages && op->ev_ok) { cudaEventRecord(op->ev[2 * PURIFY_STAGE_CROP], st); op->stage_ran[PURIFY_STAGE_CROP] = true; }
+    const long long tot = (long long)(row1 - row0) * op->n;
+    if (tot > 0) {
+        if (op->dtype == PURIFY_C64)
+            pk::crop_kernel<float><<<grid_for(tot, 256, 148 * 32), 256, 0, st>>>((const float2*)op->grid, (const float*)op->corr,
+                                                                                 (float2*)x, op->n, op->K, row0, row1);
+        else
+            pk::crop_kernel<double><<<grid_for(tot, 256, 148 * 32), 256, 0, st>>>((const double2*)op->grid, (const double*)op->corr,
+                                                                                  (double2*)x, op->n, op->K, row0, row1);
+        op->launches++;
+    }
+    if (timed && op->time_stages && op->ev_ok) cudaEventRecord(op->ev[2 * PURIFY_STAGE_CROP + 1], st);
     CK(cudaGetLastError());
     return PURIFY_OK;
 }
@@ -441,10 +458,25 @@ int launch_permute(purify_op* op, const void* in, void* out, int to_native, cuda
     return PURIFY_OK;
 }
 
-int ensure_ws(purify_op* op, void** p, size_t bytes) {
-    if (*p) return PURIFY_OK;
-    return dev_alloc(op, p, bytes);
+// lazily allocated workspace of at least `bytes` (grown when a later call needs more: the pointer may change)
+int ensure_ws(purify_op* op, void** p, size_t* have, size_t bytes) {
+    if (*p && *have >= bytes) return PURIFY_OK;
+    if (*p) {
+        cudaError_t e = cudaDeviceSynchronize();      // work enqueued on the old buffer must finish before it is freed
+        if (e != cudaSuccess) return fail(PURIFY_ERR_CUDA, "synchronise before workspace growth failed: %s", cudaGetErrorString(e));
+        cudaFree(*p);
+        op->device_bytes -= (long long)*have;
+        *p = nullptr; *have = 0;
+        op->graph_stale = true;                       // a captured graph may hold the old pointer
+    }
+    int rc = dev_alloc(op, p, bytes);
+    if (rc == PURIFY_OK) *have = bytes ? bytes : 16;
+    return rc;
 }
+#define WS_Y(op, bytes) ensure_ws(op, &(op)->y_ws, &(op)->y_ws_bytes, bytes)
+#define WS_Y2(op, bytes) ensure_ws(op, &(op)->y_ws2, &(op)->y_ws2_bytes, bytes)
+#define WS_X(op, bytes) ensure_ws(op, &(op)->x_ws, &(op)->x_ws_bytes, bytes)
+#define WS_SCAL(op) ensure_ws(op, (void**)&(op)->scal_ws, &(op)->scal_ws_bytes, sizeof(double))
 
 void begin_call(purify_op* op) {
     op->launches = 0;
@@ -833,7 +865,8 @@ int create_impl(purify_op** out, int n, int oversample, int J, long long M, cons
         if (opts->table_samples_per_unit) R = opts->table_samples_per_unit;
         if (opts->chunk) chunk = opts->chunk;
         time_stages = opts->time_stages;
-        admm_unfused = opts->reserved[0] != 0;
+        admm_unfused = opts->admm_unfused != 0;
+        if (opts->reserved[0] || opts->reserved[1]) return fail(PURIFY_ERR_INVALID_ARG, "purify_opts.reserved must be 0");
     }
     if (mode != PURIFY_KERNEL_ANALYTIC && mode != PURIFY_KERNEL_TABLE)
         return fail(PURIFY_ERR_UNSUPPORTED, "unknown kernel mode %d", mode);
@@ -868,7 +901,7 @@ int create_impl(purify_op** out, int n, int oversample, int J, long long M, cons
     if (rc) return bail(rc);
     if (dtype == PURIFY_C64) {
         rc = build_bins_x<float>(op, uv_dev, w_dev, st);
-    } else if (J <= 6 && !(opts && opts->reserved[1])) {     // reserved[1] != 0: force the tile-sorted complex128 kernels
+    } else if (J <= 6 && !(opts && opts->force_tile_sorted)) {
         rc = build_bins_x<double>(op, uv_dev, w_dev, st);
     } else {
         rc = build_bins<double>(op, uv_dev, w_dev, st);
@@ -933,6 +966,11 @@ int purify_op_destroy(purify_op* op) {
     cudaFree(op->grid); cudaFree(op->uv_s); cudaFree(op->w_s); cudaFree(op->perm); cudaFree(op->inv_perm); cudaFree(op->scal_ws); cudaFree(op->items);
     cudaFree(op->corr); cudaFree(op->table); cudaFree(op->y_ws); cudaFree(op->x_ws); cudaFree(op->y_ws2);
     cudaFree(op->x_bhdr); cudaFree(op->x_blane); cudaFree(op->x_items); cudaFree(op->x_counter);
+    for (cudaEvent_t e : op->band_ev) cudaEventDestroy(e);
+    if (op->comm_done) cudaEventDestroy(op->comm_done);
+    if (op->comm_stream) cudaStreamDestroy(op->comm_stream);
+    if (op->normal_exec) cudaGraphExecDestroy(op->normal_exec);
+    if (op->cap_stream) cudaStreamDestroy(op->cap_stream);
     if (op->plan_ok) cufftDestroy(op->plan);
     if (op->ev_ok) for (int i = 0; i < 2 * PURIFY_STAGE_COUNT; ++i) cudaEventDestroy(op->ev[i]);
     cudaGetLastError();
@@ -965,7 +1003,7 @@ static int degrid_impl(purify_op* op, const void* x, void* y, bool caller_order,
     RUN(launch_pad(op, x, st));
     RUN(launch_fft(op, CUFFT_FORWARD, st));
     if (op->batched && caller_order) {
-        RUN(ensure_ws(op, &op->y_ws, csize(op) * (size_t)op->M_native));
+        RUN(WS_Y(op, csize(op) * (size_t)op->M_native));
         RUN(launch_degrid(op, op->y_ws, false, st));
         return launch_permute(op, op->y_ws, y, 0, st);
     }
@@ -975,7 +1013,7 @@ static int degrid_impl(purify_op* op, const void* x, void* y, bool caller_order,
 
 static int grid_impl(purify_op* op, const void* y, void* x, bool caller_order, cudaStream_t st) {
     if (op->batched && caller_order) {
-        RUN(ensure_ws(op, &op->y_ws, csize(op) * (size_t)op->M_native));
+        RUN(WS_Y(op, csize(op) * (size_t)op->M_native));
         RUN(launch_permute(op, y, op->y_ws, 1, st));
         y = op->y_ws;
         caller_order = false;
@@ -1012,14 +1050,114 @@ int purify_grid_native(purify_op* op, const void* y_native_dev, void* x_dev, voi
     return grid_impl(op, y_native_dev, x_dev, false, (cudaStream_t)cuda_stream);
 }
 
+// The step of an ADMM iteration / power iteration.  Its seven launches (S+Z, F, W G, memset, G^dagger W^dagger,
+// F^dagger, Z^dagger S^dagger) are captured ONCE per (x_in, x_out) pair into a CUDA graph - on an internal stream,
+// because the caller's may be the legacy default stream, which cannot capture - and replayed on the caller's stream.
+// Stage timing needs events between the launches: with it switched on the launches are issued one by one.
+static int normal_eager(purify_op* op, const void* x_in, void* x_out, cudaStream_t st) {
+    RUN(degrid_impl(op, x_in, op->y_ws, false, st));
+    RUN(grid_impl(op, op->y_ws, x_out, false, st));
+    return PURIFY_OK;
+}
+
 int purify_normal(purify_op* op, const void* x_in_dev, void* x_out_dev, void* cuda_stream) {
     NEED_OP(op); NEED_PTR(x_in_dev, "x_in"); NEED_PTR(x_out_dev, "x_out");
     begin_call(op);
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    RUN(ensure_ws(op, &op->y_ws, csize(op) * (size_t)op->M_native));
-    RUN(degrid_impl(op, x_in_dev, op->y_ws, false, st));
-    RUN(grid_impl(op, op->y_ws, x_out_dev, false, st));
+    RUN(WS_Y(op, csize(op) * (size_t)op->M_native));
+    if (op->time_stages || op->graph_failed) return normal_eager(op, x_in_dev, x_out_dev, st);
+    if (!op->normal_exec || op->graph_stale || op->normal_in != x_in_dev || op->normal_out != x_out_dev) {
+        if (op->normal_exec) { cudaGraphExecDestroy(op->normal_exec); op->normal_exec = nullptr; }
+        if (!op->cap_stream && cudaStreamCreateWithFlags(&op->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
+            cudaGetLastError(); op->cap_stream = nullptr; op->graph_failed = true;
+            return normal_eager(op, x_in_dev, x_out_dev, st);
+        }
+        // first use of every kernel instantiation outside the capture (occupancy queries, attributes, lazy module load)
+        if (!op->normal_warm || op->graph_stale) {
+            RUN(normal_eager(op, x_in_dev, x_out_dev, st));
+            op->normal_warm = true; op->graph_stale = false;
+            return PURIFY_OK;                           // (this call is done; the next one captures)
+        }
+        cudaGraph_t g = nullptr;
+        bool ok = cudaStreamBeginCapture(op->cap_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+        int rc = PURIFY_OK;
+        if (ok) {
+            const int l0 = op->launches;
+            rc = normal_eager(op, x_in_dev, x_out_dev, op->cap_stream);
+            op->normal_launches = op->launches - l0;
+            op->launches = l0;
+            ok = cudaStreamEndCapture(op->cap_stream, &g) == cudaSuccess && rc == PURIFY_OK && g;
+        }
+        if (ok) ok = cudaGraphInstantiate(&op->normal_exec, g, 0) == cudaSuccess;
+        if (g) cudaGraphDestroy(g);
+        cufftSetStream(op->plan, st);
+        if (!ok) {                                      // no graph on this system: issue the launches one by one from now on
+            cudaGetLastError();
+            op->normal_exec = nullptr; op->graph_failed = true;
+            return normal_eager(op, x_in_dev, x_out_dev, st);
+        }
+        op->normal_in = x_in_dev; op->normal_out = x_out_dev;
+    }
+    CK(cudaGraphLaunch(op->normal_exec, st));
+    op->launches += op->normal_launches;
     return PURIFY_OK;
+}
+
+// ---- f3: the distributed-image operator (Eq. 37-38; Algorithm 2).  Every rank
+// holds its own visibilities and a replica of x; Phi needs no exchange; Phi^dagger ends with the sum over ranks of
+// the n x n images.  The exchange itself is the caller's (NCCL, MPI, ...): the library hands the image to
+// `allreduce` in `bands` horizontal bands as they leave the crop kernel - band k is being reduced on the handle's side
+// stream while band k + 1 is cropped on the caller's stream - and makes the caller's stream wait for the last one.
+static int grid_dist_tail(purify_op* op, void* x, int bands, purify_allreduce_fn allreduce, void* user, cudaStream_t st) {
+    if (bands < 1) bands = 1;
+    if (bands > op->n) bands = op->n;
+    if (!allreduce) return launch_crop(op, x, st);
+    if (!op->comm_stream) CK(cudaStreamCreateWithFlags(&op->comm_stream, cudaStreamNonBlocking));
+    if (!op->comm_done) CK(cudaEventCreateWithFlags(&op->comm_done, cudaEventDisableTiming));
+    while ((int)op->band_ev.size() < bands) {
+        cudaEvent_t e;
+        CK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        op->band_ev.push_back(e);
+    }
+    const size_t row_bytes = csize(op) * (size_t)op->n;
+    if (op->time_stages && op->ev_ok) { cudaEventRecord(op->ev[2 * PURIFY_STAGE_CROP], st); op->stage_ran[PURIFY_STAGE_CROP] = true; }
+    for (int k = 0; k < bands; ++k) {
+        const int r0 = (int)((long long)op->n * k / bands), r1 = (int)((long long)op->n * (k + 1) / bands);
+        RUN(launch_crop(op, x, st, r0, r1, false));
+        CK(cudaEventRecord(op->band_ev[k], st));
+        CK(cudaStreamWaitEvent(op->comm_stream, op->band_ev[k], 0));
+        const int rc = allreduce(user, (char*)x + row_bytes * (size_t)r0, (long long)(r1 - r0) * op->n * 2,
+                                 op->dtype == PURIFY_C128, (void*)op->comm_stream);
+        if (rc != 0) return fail(PURIFY_ERR_CUDA, "the all-reduce callback failed on band %d (returned %d)", k, rc);
+    }
+    CK(cudaEventRecord(op->comm_done, op->comm_stream));
+    CK(cudaStreamWaitEvent(st, op->comm_done, 0));
+    if (op->time_stages && op->ev_ok) cudaEventRecord(op->ev[2 * PURIFY_STAGE_CROP + 1], st);      // crop + exchange
+    return PURIFY_OK;
+}
+
+int purify_grid_dist(purify_op* op, const void* y_native_dev, void* x_dev, int bands, purify_allreduce_fn allreduce,
+                     void* user, void* cuda_stream) {
+    NEED_OP(op); NEED_PTR(x_dev, "x"); if (op->M > 0) NEED_PTR(y_native_dev, "y");
+    if (op->batched && ((uintptr_t)y_native_dev & 15u))
+        return fail(PURIFY_ERR_INVALID_ARG, "y_native must be 16-byte aligned for the batched layout");
+    begin_call(op);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    RUN(launch_grid(op, y_native_dev, false, st));
+    RUN(launch_fft(op, CUFFT_INVERSE, st));
+    return grid_dist_tail(op, x_dev, bands, allreduce, user, st);
+}
+
+int purify_normal_dist(purify_op* op, const void* x_in_dev, void* x_out_dev, int bands, purify_allreduce_fn allreduce,
+                       void* user, void* cuda_stream) {
+    NEED_OP(op); NEED_PTR(x_in_dev, "x_in"); NEED_PTR(x_out_dev, "x_out");
+    begin_call(op);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    RUN(WS_Y(op, csize(op) * (size_t)op->M_native));
+    RUN(degrid_impl(op, x_in_dev, op->y_ws, false, st));
+    RUN(launch_grid(op, op->y_ws, false, st));
+    RUN(launch_fft(op, CUFFT_INVERSE, st));
+    return grid_dist_tail(op, x_out_dev, bands, allreduce, user, st);
 }
 
 int purify_permute_to_native(purify_op* op, const void* y_caller_dev, void* y_native_dev, void* cuda_stream) {
@@ -1040,8 +1178,8 @@ int purify_degrid_host(purify_op* op, const void* x_host, void* y_host, void* cu
     begin_call(op);
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t xb = csize(op) * (size_t)op->n * op->n, yb = csize(op) * (size_t)op->M;
-    RUN(ensure_ws(op, &op->x_ws, xb));
-    RUN(ensure_ws(op, &op->y_ws2, yb));
+    RUN(WS_X(op, xb));
+    RUN(WS_Y2(op, yb));
     CK(cudaMemcpyAsync(op->x_ws, x_host, xb, cudaMemcpyHostToDevice, st));
     RUN(degrid_impl(op, op->x_ws, op->y_ws2, true, st));
     if (yb) CK(cudaMemcpyAsync(y_host, op->y_ws2, yb, cudaMemcpyDeviceToHost, st));
@@ -1054,8 +1192,8 @@ int purify_grid_host(purify_op* op, const void* y_host, void* x_host, void* cuda
     begin_call(op);
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t xb = csize(op) * (size_t)op->n * op->n, yb = csize(op) * (size_t)op->M;
-    RUN(ensure_ws(op, &op->x_ws, xb));
-    RUN(ensure_ws(op, &op->y_ws2, yb));
+    RUN(WS_X(op, xb));
+    RUN(WS_Y2(op, yb));
     if (yb) CK(cudaMemcpyAsync(op->y_ws2, y_host, yb, cudaMemcpyHostToDevice, st));
     RUN(grid_impl(op, op->y_ws2, op->x_ws, true, st));
     CK(cudaMemcpyAsync(x_host, op->x_ws, xb, cudaMemcpyDeviceToHost, st));
@@ -1068,8 +1206,8 @@ int purify_normal_host(purify_op* op, const void* x_in_host, void* x_out_host, v
     begin_call(op);
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t xb = csize(op) * (size_t)op->n * op->n;
-    RUN(ensure_ws(op, &op->x_ws, xb));
-    RUN(ensure_ws(op, &op->y_ws, csize(op) * (size_t)op->M_native));
+    RUN(WS_X(op, xb));
+    RUN(WS_Y(op, csize(op) * (size_t)op->M_native));
     CK(cudaMemcpyAsync(op->x_ws, x_in_host, xb, cudaMemcpyHostToDevice, st));
     RUN(degrid_impl(op, op->x_ws, op->y_ws, false, st));
     RUN(grid_impl(op, op->y_ws, op->x_ws, false, st));
@@ -1088,9 +1226,9 @@ int purify_op_norm(purify_op* op, const void* x0_dev, int max_iter, double rel_t
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const long long N = (long long)op->n * op->n;
     const size_t xb = csize(op) * (size_t)N;
-    RUN(ensure_ws(op, &op->x_ws, xb));
-    RUN(ensure_ws(op, &op->y_ws, csize(op) * (size_t)op->M_native));
-    RUN(ensure_ws(op, (void**)&op->scal_ws, sizeof(double)));
+    RUN(WS_X(op, xb));
+    RUN(WS_Y(op, csize(op) * (size_t)op->M_native));
+    RUN(WS_SCAL(op));
     const bool f32 = op->dtype == PURIFY_C64;
     auto norm2 = [&](const void* v, double* host) -> int {
         CK(cudaMemsetAsync(op->scal_ws, 0, sizeof(double), st));
@@ -1148,9 +1286,8 @@ int purify_admm_fidelity_step(purify_op* op, const void* x_dev, const void* y_na
     begin_call(op);
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const long long Mn = op->M_native;
-    RUN(ensure_ws(op, &op->y_ws, csize(op) * (size_t)Mn));
-    RUN(ensure_ws(op, &op->y_ws2, csize(op) * (size_t)(Mn > op->M ? Mn : op->M)));
-    RUN(ensure_ws(op, (void**)&op->scal_ws, sizeof(double)));
+    RUN(WS_Y(op, csize(op) * (size_t)Mn));
+    RUN(WS_SCAL(op));
     if (op->batched && op->dtype == PURIFY_C64 && op->mode == PURIFY_KERNEL_ANALYTIC && !op->admm_unfused) {
         // fused form: the norm is accumulated inside the degridding kernel, r / s_new / z are formed slot by slot inside
         // the gridding kernel (z is never stored); two passes over the M-sized vectors less than the unfused form below
@@ -1172,6 +1309,7 @@ int purify_admm_fidelity_step(purify_op* op, const void* x_dev, const void* y_na
         }
         return PURIFY_OK;
     }
+    RUN(WS_Y2(op, csize(op) * (size_t)(Mn > op->M ? Mn : op->M)));      // z = v - r + s_new, M_native entries
     const unsigned* pm = op->batched ? op->perm : nullptr;     // padding mask (batched layout only)
     // line 3: v = Phi x
     RUN(degrid_impl(op, x_dev, op->y_ws, false, st));
@@ -1235,7 +1373,7 @@ int purify_stage_gridded(purify_op* op, const void* y_dev, void* B_dev, void* cu
     begin_call(op);
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (op->batched) {
-        RUN(ensure_ws(op, &op->y_ws, csize(op) * (size_t)op->M_native));
+        RUN(WS_Y(op, csize(op) * (size_t)op->M_native));
         RUN(launch_permute(op, y_dev, op->y_ws, 1, st));
         RUN(launch_grid(op, op->y_ws, false, st));
     } else {
@@ -1254,7 +1392,58 @@ int purify_stage_times_ms(const purify_op* op, float out[PURIFY_STAGE_COUNT]) {
     return PURIFY_OK;
 }
 
+int purify_op_set_time_stages(purify_op* op, int enable) {
+    NEED_OP(op);
+    op->time_stages = enable != 0;
+    return PURIFY_OK;
+}
+
 int purify_last_launch_count(const purify_op* op) { return op ? op->launches : 0; }
+
+// ---- issue-rate probe of the packed fp32 instruction forms (csrc/ubench.cuh)
+int purify_ubench_fma(int form, int warps_per_sm, double* cycles_per_instr_out, double* sm_ghz_out) {
+    NEED_PTR(cycles_per_instr_out, "cycles_per_instr_out");
+    if (form < 0 || form > 4) return fail(PURIFY_ERR_INVALID_ARG, "form must be in [0, 4] (got %d)", form);
+    if (warps_per_sm < 4 || warps_per_sm > 32 || (warps_per_sm & 3)) return fail(PURIFY_ERR_INVALID_ARG, "warps_per_sm must be 4, 8, ..., 32");
+    RUN(check_device());
+    int dev = 0, sms = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    float* out = nullptr; long long* cyc = nullptr;
+    CK(cudaMalloc(&out, sizeof(float) * (size_t)sms * 1024));
+    if (cudaMalloc(&cyc, sizeof(long long) * (size_t)sms) != cudaSuccess) { cudaFree(out); cudaGetLastError(); return fail(PURIFY_ERR_ALLOC, "cudaMalloc failed"); }
+    const int iters = 4000, threads = warps_per_sm * 32;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    auto launch = [&](int n) {
+        switch (form) {
+            case 0: pk::ubench_fma_kernel<0><<<sms, threads>>>(out, cyc, n, 1.0001f, 0.3f); break;
+            case 1: pk::ubench_fma_kernel<1><<<sms, threads>>>(out, cyc, n, 1.0001f, 0.3f); break;
+            case 2: pk::ubench_fma_kernel<2><<<sms, threads>>>(out, cyc, n, 1.0001f, 0.3f); break;
+            case 3: pk::ubench_fma_kernel<3><<<sms, threads>>>(out, cyc, n, 1.0001f, 0.3f); break;
+            default: pk::ubench_fma_kernel<4><<<sms, threads>>>(out, cyc, n, 1.0001f, 0.3f); break;
+        }
+    };
+    launch(10);
+    cudaEventRecord(e0);
+    launch(iters);
+    cudaEventRecord(e1);
+    cudaError_t e = cudaEventSynchronize(e1);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    std::vector<long long> h((size_t)sms);
+    if (e == cudaSuccess) e = cudaMemcpy(h.data(), cyc, sizeof(long long) * (size_t)sms, cudaMemcpyDeviceToHost);
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(out); cudaFree(cyc);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(PURIFY_ERR_CUDA, "ubench failed: %s", cudaGetErrorString(e)); }
+    double c = 0;
+    for (int i = 0; i < sms; ++i) c += (double)h[i];
+    c /= sms;
+    // instructions per SM sub-partition: every warp issues iters x REP x NA instructions (form 0: two scalar FFMA each)
+    const double per_smsp = (double)iters * pk::UB_REP * pk::UB_NA * (form == 0 ? 2.0 : 1.0) * (warps_per_sm / 4.0);
+    *cycles_per_instr_out = c / per_smsp;
+    if (sm_ghz_out) *sm_ghz_out = ms > 0.f ? c / (ms * 1e6) : 0.0;
+    return PURIFY_OK;
+}
 
 const char* purify_strerror(int status) {
     switch (status) {

@@ -12,7 +12,7 @@ import os
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("PURIFY_OP_LIB") or os.path.join(_HERE, "libpurify_op.so")   # env override: tuning builds
+LIB_PATH = os.path.join(_HERE, "libpurify_op.so")
 
 C64, C128 = 0, 1
 ANALYTIC, TABLE = 0, 1
@@ -25,13 +25,15 @@ SYMBOLS = (
     "purify_degrid_native", "purify_grid_native", "purify_permute_to_native",
     "purify_permute_from_native", "purify_degrid_host", "purify_grid_host", "purify_normal_host",
     "purify_stage_fourier_grid", "purify_stage_gridded", "purify_stage_times_ms",
-    "purify_last_launch_count", "purify_strerror", "purify_last_error", "purify_version", "purify_op_norm", "purify_admm_fidelity_step",
+    "purify_last_launch_count", "purify_strerror", "purify_last_error", "purify_version", "purify_op_norm",
+    "purify_admm_fidelity_step", "purify_op_set_time_stages", "purify_ubench_fma", "purify_grid_dist", "purify_normal_dist",
 )
 
 
 class PurifyOpts(C.Structure):
     _fields_ = [("kernel_mode", C.c_int), ("table_samples_per_unit", C.c_int), ("chunk", C.c_int),
-                ("time_stages", C.c_int), ("reserved", C.c_int * 4)]
+                ("time_stages", C.c_int), ("admm_unfused", C.c_int), ("force_tile_sorted", C.c_int),
+                ("reserved", C.c_int * 2)]
 
 
 class PurifyInfo(C.Structure):
@@ -40,6 +42,9 @@ class PurifyInfo(C.Structure):
                 ("n_tiles_nonempty", C.c_int), ("n_items", C.c_int), ("poly_degree", C.c_int),
                 ("poly_max_abs_err", C.c_double), ("device_bytes", C.c_longlong), ("max_tile_count", C.c_longlong),
                 ("M_native", C.c_longlong), ("n_batches", C.c_longlong), ("layout", C.c_int), ("tile_h", C.c_int)]
+
+
+ALLREDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_longlong, C.c_int, C.c_void_p)
 
 
 class PurifyError(RuntimeError):
@@ -76,7 +81,14 @@ def load_library():
     L.purify_op_norm.restype = ip
     L.purify_admm_fidelity_step.argtypes = [vp, vp, vp, vp, C.c_double, C.c_double, vp, C.POINTER(C.c_double), vp]
     L.purify_admm_fidelity_step.restype = ip
+    for name in ("purify_grid_dist", "purify_normal_dist"):
+        getattr(L, name).argtypes = [vp, vp, vp, ip, ALLREDUCE_FN, vp, vp]
+        getattr(L, name).restype = ip
+    L.purify_ubench_fma.argtypes = [ip, ip, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    L.purify_ubench_fma.restype = ip
     L.purify_stage_times_ms.argtypes = [vp, C.POINTER(C.c_float)]
+    L.purify_op_set_time_stages.argtypes = [vp, ip]
+    L.purify_op_set_time_stages.restype = ip
     L.purify_last_launch_count.argtypes = [vp]
     L.purify_strerror.argtypes = [ip]
     L.purify_strerror.restype = C.c_char_p
@@ -109,9 +121,8 @@ class PurifyOp:
         self._L = load_library()
         self._h = C.c_void_p()
         self.n, self.K, self.J, self.dtype = int(n), 2 * int(n), int(J), int(dtype)
-        opts = PurifyOpts(int(kernel_mode), int(table_samples_per_unit), int(chunk), int(bool(time_stages)))
-        opts.reserved[0] = int(bool(admm_unfused))     # purify_admm_fidelity_step: separate norm / update kernels
-        opts.reserved[1] = int(bool(tile_sorted))      # complex128: the tile-sorted kernels instead of the batched layout
+        opts = PurifyOpts(int(kernel_mode), int(table_samples_per_unit), int(chunk), int(bool(time_stages)),
+                          int(bool(admm_unfused)), int(bool(tile_sorted)))
         M = 0 if uv is None else int(uv.shape[0])
         self.M = M
         rdt = _RDT.get(self.dtype, torch.float32)
@@ -173,6 +184,9 @@ class PurifyOp:
         _check(self._L.purify_stage_times_ms(self._h, arr), "purify_stage_times_ms")
         return {STAGES[i]: float(arr[i]) for i in range(8)}
 
+    def set_time_stages(self, enable: bool):
+        _check(self._L.purify_op_set_time_stages(self._h, int(bool(enable))), "purify_op_set_time_stages")
+
     def last_launch_count(self) -> int:
         return int(self._L.purify_last_launch_count(self._h))
 
@@ -219,6 +233,42 @@ class PurifyOp:
         out = self._new_x() if out is None else out
         self._dev(x, out)
         _check(self._L.purify_normal(self._h, self._x(x), self._x(out, "out"), _stream()), "purify_normal")
+        return out
+
+    # -- f3: distributed-image operator; `allreduce(band: torch.Tensor)` sums a real view of one image band over the ranks
+    def _dist_cb(self, out, allreduce):
+        """ctypes callback that turns (pointer, count, stream) into a tensor view of `out` on that stream."""
+        if allreduce is None:
+            return C.cast(None, ALLREDUCE_FN)
+        flat = torch.view_as_real(out).reshape(-1)
+        base, item = flat.data_ptr(), flat.element_size()
+
+        def cb(_user, ptr, count, _is_double, stream):
+            try:
+                off = (int(ptr) - base) // item
+                with torch.cuda.stream(torch.cuda.ExternalStream(int(stream or 0))):
+                    allreduce(flat[off:off + int(count)])
+                return 0
+            except Exception:           # never let an exception cross the C boundary
+                import traceback
+                traceback.print_exc()
+                return 1
+        return ALLREDUCE_FN(cb)
+
+    def grid_dist(self, y_native, x=None, allreduce=None, bands: int = 4):
+        x = self._new_x() if x is None else x
+        self._dev(x, y_native)
+        cb = self._dist_cb(x, allreduce)
+        _check(self._L.purify_grid_dist(self._h, self._y(y_native, "y_native", True), self._x(x), int(bands), cb, None, _stream()),
+               "purify_grid_dist")
+        return x
+
+    def normal_dist(self, x, out=None, allreduce=None, bands: int = 4):
+        out = self._new_x() if out is None else out
+        self._dev(x, out)
+        cb = self._dist_cb(out, allreduce)
+        _check(self._L.purify_normal_dist(self._h, self._x(x), self._x(out, "out"), int(bands), cb, None, _stream()),
+               "purify_normal_dist")
         return out
 
     def permute_to_native(self, y, out=None):
@@ -283,6 +333,19 @@ class PurifyOp:
         _check(self._L.purify_stage_gridded(self._h, self._y(y), C.c_void_p(B.data_ptr()), _stream()),
                "purify_stage_gridded")
         return B
+
+
+UBENCH_FORMS = ("2 x FFMA, 3 registers", "FFMA2 broadcast scalar x pair + pair (degridding row pass)",
+                "FFMA2 pair x pair + pair (weight combination)", "FFMA2 pair x pair + constant (Horner step)",
+                "FFMA2 varying scalar x shared pair + pair (gridding)")
+
+
+def ubench_fma(form: int, warps_per_sm: int = 16):
+    """(SM cycles per warp instruction per SM sub-partition, SM clock in GHz) of one packed-fp32 instruction form."""
+    L = load_library()
+    cyc, ghz = C.c_double(0.0), C.c_double(0.0)
+    _check(L.purify_ubench_fma(int(form), int(warps_per_sm), C.byref(cyc), C.byref(ghz)), "purify_ubench_fma")
+    return float(cyc.value), float(ghz.value)
 
 
 class _DeviceArray:

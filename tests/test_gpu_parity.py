@@ -9,10 +9,15 @@ import torch
 
 import oracle
 from inputs import synth
+from parity_util import compare
 
 pytestmark = pytest.mark.gpu
 
 TOL = {"c128": 1e-12, "c64": 1e-5}
+# Composite operators (Phi^dagger Phi, the ADMM data-fidelity step, its residual norm) get NO multiple of the tolerance:
+# measured, they stay below 0.09 tol (profiles/parity_r2.md).
+ADMM_FACTOR = 1.0
+ADMM_NORM_FACTOR = 1.0
 
 
 def rel_l2(a, b):
@@ -48,7 +53,8 @@ def cast_problem(x, uv, w, dtype):
 
 
 def run_all_checks(x, uv, w, J, dtype, mode="analytic", R=4096, **kw):
-    """degrid (caller + native order), grid (both orders), normal, stages - all against the oracle."""
+    """degrid (caller + native order), grid (both orders), normal, stages - all against the oracle, rel-L2 over the
+    whole output AND the largest element-wise deviation (parity_util.compare)."""
     from paper_1903_04502_b200 import ANALYTIC, TABLE
     n = x.shape[0]
     tol = TOL[dtype]
@@ -57,32 +63,33 @@ def run_all_checks(x, uv, w, J, dtype, mode="analytic", R=4096, **kw):
     op = make_op(n, J, uv, w, dtype, kernel_mode=TABLE if mode == "table" else ANALYTIC,
                  table_samples_per_unit=R if mode == "table" else 0, **kw)
     okw = dict(mode=mode, R=R, idx_prec=idx_prec(dtype))
+    ctx = dict(n=n, J=J, M=M, dtype=dtype, mode=mode)
     # ---- Phi
     y_ref = oracle.degrid(x, uv, w, J, **okw)
     y = host(op.degrid(dev(x)))
-    assert rel_l2(y, y_ref) <= tol
+    compare("Phi caller order", y, y_ref, tol, **ctx)
     perm = host(op.permutation())                          # M_native entries, -1 = padding (complex64 layout)
     valid = perm >= 0
     assert len(perm) == op.M_native >= M
     assert sorted(perm[valid].tolist()) == list(range(M))
     y_nat = host(op.degrid(dev(x), native=True))
-    assert rel_l2(y_nat[valid], y_ref[perm[valid]]) <= tol
+    compare("Phi native order", y_nat[valid], y_ref[perm[valid]], tol, **ctx)
     assert np.array_equal(y_nat[valid], y[perm[valid]])     # same numbers, different order
     assert not np.any(y_nat[~valid])                        # padding entries are written as 0
     # stage: Fourier grid in the mathematical layout
     B_ref = oracle.fft2(oracle.pad(x, J), -1)
-    assert rel_l2(host(op.stage_fourier_grid(dev(x))), B_ref) <= tol
+    compare("F Z S x", host(op.stage_fourier_grid(dev(x))), B_ref, tol, **ctx)
     # ---- Phi^dagger on random data (caller order and native order)
     yv = synth.random_complex((M,), seed=77, dtype=dtype)
     img_ref = oracle.grid(yv, uv, w, n, J, **okw)
     img = host(op.grid(dev(yv)))
-    assert rel_l2(img, img_ref) <= tol
+    compare("Phi^dagger caller order", img, img_ref, tol, **ctx)
     yv_nat = np.full(len(perm), np.nan + 1j * np.nan, dtype=yv.dtype)     # padding holds NaN: must be ignored
     yv_nat[valid] = yv[perm[valid]]
     img_nat = host(op.grid(dev(yv_nat), native=True))
-    assert rel_l2(img_nat, img_ref) <= tol
+    compare("Phi^dagger native order", img_nat, img_ref, tol, **ctx)
     Bp_ref = oracle.grid_to_grid(yv, uv, w, 2 * n, J, **okw)
-    assert rel_l2(host(op.stage_gridded(dev(yv))), Bp_ref) <= tol
+    compare("G^dagger W^dagger y", host(op.stage_gridded(dev(yv))), Bp_ref, tol, **ctx)
     # permutation helpers
     to_nat = host(op.permute_to_native(dev(yv)))
     assert np.array_equal(to_nat[valid], yv[perm[valid]]) and not np.any(to_nat[~valid])
@@ -91,23 +98,25 @@ def run_all_checks(x, uv, w, J, dtype, mode="analytic", R=4096, **kw):
     nrm_ref = oracle.grid(y_ref, uv, w, n, J, **okw)
     xin = dev(x)
     nrm = host(op.normal(xin))
-    assert rel_l2(nrm, nrm_ref) <= 2 * tol
+    compare("Phi^dagger Phi", nrm, nrm_ref, tol, **ctx)
+    for _ in range(3):                                     # replayed from the CUDA graph: the same result
+        compare("Phi^dagger Phi (graph replay)", host(op.normal(xin)), nrm_ref, tol, **ctx)
     # in place
     op.normal(xin, out=xin)
-    assert rel_l2(host(xin), nrm_ref) <= 2 * tol
+    compare("Phi^dagger Phi in place", host(xin), nrm_ref, tol, **ctx)
     # ---- adjoint identity evaluated with GPU results
     xr = synth.random_complex((n, n), seed=78, dtype=dtype)
     Px = host(op.degrid(dev(xr))).astype(np.complex128)
     Pty = img.astype(np.complex128)
     lhs, rhs = np.vdot(Px, yv.astype(np.complex128)), np.vdot(xr.astype(np.complex128), Pty)
-    assert abs(lhs - rhs) / (np.linalg.norm(Px) * np.linalg.norm(yv)) <= 10 * tol
+    assert abs(lhs - rhs) / (np.linalg.norm(Px) * np.linalg.norm(yv)) <= tol
     # ---- host-buffer entry points give the same numbers
     yh = op.degrid_host(torch.from_numpy(x).pin_memory()).numpy()
     assert np.array_equal(yh, y)
     nh = op.normal_host(torch.from_numpy(x).pin_memory()).numpy()
-    assert rel_l2(nh, nrm_ref) <= 2 * tol
+    compare("Phi^dagger Phi host buffers", nh, nrm_ref, tol, **ctx)
     gh = op.grid_host(torch.from_numpy(yv).pin_memory()).numpy()
-    assert rel_l2(gh, img_ref) <= tol
+    compare("Phi^dagger host buffers", gh, img_ref, tol, **ctx)
     info = op.info()
     op.close()
     return info
@@ -149,7 +158,7 @@ def test_config2_noisy_data_adjoint():
     y = synth.add_noise(y0, 30.0, cfg.seed)
     assert np.linalg.norm(y - y0) / np.linalg.norm(y0) == pytest.approx(10 ** (-30 / 20), rel=0.02)
     op = make_op(cfg.n, 4, uv, w, "c128")
-    assert rel_l2(host(op.grid(dev(y))), oracle.grid(y, uv, w, cfg.n, 4)) <= TOL["c128"]
+    compare("Phi^dagger on noisy data", host(op.grid(dev(y))), oracle.grid(y, uv, w, cfg.n, 4), TOL["c128"], n=cfg.n, J=4, M=len(uv), dtype="c128")
     op.close()
 
 
@@ -302,7 +311,7 @@ def test_operator_norm_power_method(dtype):
     x0 = synth.random_complex((cfg.n, cfg.n), seed=21, dtype=dtype)
     _, uvc, wc = cast_problem(x, uv, w, dtype)
     op = make_op(cfg.n, cfg.J, uvc, wc, dtype)
-    tol = 1e-5 if dtype == "c64" else 1e-11
+    tol = TOL[dtype]
     for iters in (1, 7):
         lam_ref, _ = oracle.power_method(x0, uvc, wc, cfg.n, cfg.J, max_iter=iters, rel_tol=0.0, idx_prec=idx_prec(dtype))
         lam, its = op.norm(dev(x0), max_iter=iters, rel_tol=0.0)
@@ -343,11 +352,39 @@ def test_admm_fidelity_step(dtype, unfused, case):
     s_dev = dev(s_nat)
     g, nrm = op.admm_fidelity_step(dev(x), dev(y_nat), s_dev, eps, 0.9)
     tol = TOL[dtype]
-    assert abs(nrm - nrm_ref) <= 10 * tol * nrm_ref
-    assert rel_l2(host(g), g_ref) <= 4 * tol
+    ctx = dict(n=cfg.n, J=6, M=M, dtype=dtype, case=case, unfused=unfused)
+    assert abs(nrm - nrm_ref) <= ADMM_NORM_FACTOR * tol * nrm_ref
+    compare("ADMM g", host(g), g_ref, tol, l2_factor=ADMM_FACTOR, **ctx)
     s_out = host(s_dev)
-    assert rel_l2(s_out[valid], s_ref[perm[valid]]) <= 4 * tol
+    compare("ADMM s_new", s_out[valid], s_ref[perm[valid]], tol, l2_factor=ADMM_FACTOR, **ctx)
     assert not np.any(s_out[~valid])
+    op.close()
+
+
+@pytest.mark.parametrize("dtype", ["c64", "c128"])
+def test_workspace_reuse_host_call_then_unfused_admm(dtype):
+    """One handle: a host-buffer call (allocates the caller-order staging vector, M entries) followed by the unfused ADMM
+    step (needs M_native >= M entries of the same workspace): the workspace must grow, not overflow."""
+    cfg, x, uv, w = synth.make_problem(2, M=30000, J=6)
+    x, uv, w = cast_problem(x, uv, w, dtype)
+    M = len(uv)
+    op = make_op(cfg.n, 6, uv, w, dtype, admm_unfused=True)
+    assert op.M_native > M
+    yh = op.degrid_host(torch.from_numpy(x).pin_memory()).numpy()
+    y = synth.random_complex((M,), seed=51, dtype=dtype)
+    s = (synth.random_complex((M,), seed=52, dtype=dtype) * 0.25).astype(y.dtype)
+    eps = 0.4 * float(np.linalg.norm(yh + s - y))
+    g_ref, s_ref, _, nrm_ref = oracle.admm_fidelity_step(x, y, s, uv, w, cfg.n, 6, eps, 0.9, idx_prec=idx_prec(dtype))
+    perm = host(op.permutation())
+    valid = perm >= 0
+    y_nat = np.zeros(len(perm), dtype=y.dtype)
+    s_nat = np.zeros(len(perm), dtype=y.dtype)
+    y_nat[valid], s_nat[valid] = y[perm[valid]], s[perm[valid]]
+    guard = torch.full((1 << 16,), 7.0, dtype=torch.float32, device="cuda")      # something to trample on, if it did overflow
+    g, nrm = op.admm_fidelity_step(dev(x), dev(y_nat), dev(s_nat), eps, 0.9)
+    compare("ADMM g after a host call", host(g), g_ref, TOL[dtype], l2_factor=ADMM_FACTOR, n=cfg.n, J=6, M=M, dtype=dtype)
+    assert float(guard.min()) == 7.0 and float(guard.max()) == 7.0
+    assert np.array_equal(op.degrid_host(torch.from_numpy(x).pin_memory()).numpy(), yh)
     op.close()
 
 
@@ -377,13 +414,14 @@ def test_fuzz_batched_layout(seed):
     valid = perm >= 0
     assert sorted(perm[valid].tolist()) == list(range(M))
     y_ref = oracle.degrid(x, uv, w, J, idx_prec=32)
+    ctx = dict(n=n, J=J, M=M, dtype="c64", seed=seed)
     y_nat = host(op.degrid(dev(x), native=True))
-    assert rel_l2(y_nat[valid], y_ref[perm[valid]]) <= 1e-5
+    compare("fuzz Phi", y_nat[valid], y_ref[perm[valid]], 1e-5, **ctx)
     yv = synth.random_complex((M,), seed=100 + seed, dtype="c64")
     img_ref = oracle.grid(yv, uv, w, n, J, idx_prec=32)
     yv_nat = np.zeros(len(perm), dtype=np.complex64)
     yv_nat[valid] = yv[perm[valid]]
-    assert rel_l2(host(op.grid(dev(yv_nat), native=True)), img_ref) <= 1e-5
+    compare("fuzz Phi^dagger", host(op.grid(dev(yv_nat), native=True)), img_ref, 1e-5, **ctx)
     s = (synth.random_complex((M,), seed=200 + seed, dtype="c64") * np.float32(0.3)).astype(np.complex64)
     eps = 0.5 * float(np.linalg.norm(y_ref + s - yv))
     g_ref, s_ref, _, nrm_ref = oracle.admm_fidelity_step(x, yv, s, uv, w, n, J, eps, 0.7, idx_prec=32)
@@ -391,6 +429,19 @@ def test_fuzz_batched_layout(seed):
     s_nat[valid] = s[perm[valid]]
     s_dev = dev(s_nat)
     g, nrm = op.admm_fidelity_step(dev(x), dev(yv_nat), s_dev, eps, 0.7)
-    assert abs(nrm - nrm_ref) <= 1e-4 * nrm_ref
-    assert rel_l2(host(g), g_ref) <= 4e-5 and rel_l2(host(s_dev)[valid], s_ref[perm[valid]]) <= 4e-5
+    assert abs(nrm - nrm_ref) <= ADMM_NORM_FACTOR * 1e-5 * nrm_ref
+    compare("fuzz ADMM g", host(g), g_ref, 1e-5, l2_factor=ADMM_FACTOR, **ctx)
+    compare("fuzz ADMM s_new", host(s_dev)[valid], s_ref[perm[valid]], 1e-5, l2_factor=ADMM_FACTOR, **ctx)
     op.close()
+
+
+def test_ubench_fma_forms():
+    """The committed issue-rate probe (csrc/ubench.cuh) behind DESIGN.md 5's 'which roofline binds': it runs, and the
+    ordering it is quoted for holds - a Horner step (one register pair read) issues at the FMA pipe's rate of one
+    packed instruction per 2 cycles per sub-partition, the degridding row-pass form (two register pairs read) needs more."""
+    from paper_1903_04502_b200 import UBENCH_FORMS, ubench_fma
+    rates = [ubench_fma(f, 16)[0] for f in range(len(UBENCH_FORMS))]
+    assert all(0.9 < r < 8.0 for r in rates), rates
+    assert 1.9 <= rates[3] <= 2.2, rates                 # Horner form: pipe-bound
+    assert rates[1] >= rates[3] * 1.05, rates            # row-pass form: operand-bound
+    assert rates[4] <= rates[1], rates                   # gridding form is the cheaper of the two MAC forms

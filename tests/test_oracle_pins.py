@@ -209,6 +209,10 @@ def test_adjoint_identity(J, mode):
     yv = synth.random_complex((M,), seed=22)
     rng = synth.rng_for(23, 0)
     uv = rng.uniform(-K / 2, K / 2, size=(M, 2))         # includes wrapped taps
+    # R7: integer and half-integer coordinates (ties of the tap rule), alone and mixed with continuous ones
+    uv[:200] = rng.integers(-K // 2, K // 2, size=(200, 2))
+    uv[200:400] = rng.integers(-K, K, size=(200, 2)) * 0.5
+    uv[400:500, 0] = rng.integers(-K // 2, K // 2, size=100)
     w = rng.uniform(0.5, 1.5, size=M)
     Px = oracle.degrid(x, uv, w, J, mode=mode)
     Pty = oracle.grid(yv, uv, w, n, J, mode=mode)
@@ -246,6 +250,40 @@ def test_grid_footprint_and_tie_break():
     # kept tie tap has weight 1/I0(beta), not zero
     Bp = oracle.grid_to_grid(np.array([1.0 + 0j]), np.array([[6.0, 2.0]]), None, K, J)
     assert abs(Bp[2, 8]) == pytest.approx(1.0 / scipy.special.i0(2.34 * J), rel=1e-12)
+
+
+@pytest.mark.parametrize("J", [4, 6, 8])
+def test_degrid_footprint_and_tie_break_on_one_hot_grid(J):
+    """R7 for W G on its own (not through G^dagger): with a one-hot Fourier grid B = e_(r,c) the degridded value is
+    g(v - r) g(u - c) when (r, c) is one of the J x J taps - the integers in (v - J/2, v + J/2] x (u - J/2, u + J/2] -
+    and 0 otherwise.  Integer, half-integer and generic coordinates; the tap set is written out here from the
+    definition, the weights from scipy's I0."""
+    K = 32
+    beta = 2.34 * J
+
+    def g(d):
+        return float(scipy.special.i0(beta * math.sqrt(max(0.0, 1 - (2 * d / J) ** 2))) / scipy.special.i0(beta)) if abs(d) <= J / 2 else 0.0
+
+    for u, v in [(5.0, -3.0), (6.5, 2.0), (-2.0, 7.5), (0.0, 0.0), (3.25, -4.75), (-7.5, -7.5)]:
+        taps_x = [c for c in range(-K, K) if u - J / 2 < c <= u + J / 2]
+        taps_y = [r for r in range(-K, K) if v - J / 2 < r <= v + J / 2]
+        assert len(taps_x) == J and len(taps_y) == J
+        for r in range(int(math.floor(v)) - J, int(math.floor(v)) + J + 1):
+            for c in range(int(math.floor(u)) - J, int(math.floor(u)) + J + 1):
+                B = np.zeros((K, K), complex)
+                B[r % K, c % K] = 1.0
+                y = oracle.degrid_from_grid(B, np.array([[u, v]]), None, J)[0]
+                if r in taps_y and c in taps_x:
+                    assert y == pytest.approx(g(v - r) * g(u - c), rel=1e-12, abs=1e-300), (u, v, r, c)
+                else:
+                    assert y == 0.0, (u, v, r, c)
+    # the kept tie tap (distance exactly -J/2 from an integer u) carries 1/I0(beta), the dropped one (+J/2) nothing
+    B = np.zeros((K, K), complex)
+    B[2 % K, (6 + J // 2) % K] = 1.0
+    assert oracle.degrid_from_grid(B, np.array([[6.0, 2.0]]), None, J)[0].real == pytest.approx(1.0 / scipy.special.i0(beta), rel=1e-12)
+    B[:] = 0
+    B[2 % K, (6 - J // 2) % K] = 1.0
+    assert oracle.degrid_from_grid(B, np.array([[6.0, 2.0]]), None, J)[0] == 0.0
 
 
 def test_stage_consistency_and_linearity(tiny):
@@ -325,6 +363,44 @@ def test_table_index_precision_flag():
     for c in range(1233, 1237):
         assert oracle.kernel_weight(float(u32), c, J, "table", R, 32) == \
             oracle.kernel_weight(float(u32), c, J, "table", R, 64)
+
+
+def test_table_index_fp32_branch_vs_exact_arithmetic():
+    """R11, idx_prec = 32 (the branch the oracle takes for complex64 problems so that both sides decide the index in
+    the storage precision).  Where every fp32 step is exact - u an f32 number with |u| >= 1, c an integer within J/2 + 1
+    of it, R a power of two - the fp32 index must equal the index computed in exact rational arithmetic, and hence the
+    fp64 branch; 1e5 random f32 coordinates over the range of config 5 (K = 8192).  At a density that is not a power of
+    two (R = 1000) the fp32 product rounds: the two precisions may then differ by one sample on a small fraction of
+    the inputs (reported in DESIGN.md R11) and never by more."""
+    from fractions import Fraction
+    rng = synth.rng_for(77, synth.STREAM_TEST)
+    n = 100_000
+    mag = np.exp(rng.uniform(0.0, math.log(4090.0), size=n))
+    u = (mag * rng.choice([-1.0, 1.0], size=n)).astype(np.float32)
+    u[np.abs(u) < 1.0] = np.float32(1.0)
+    u[:1000] = np.round(u[:1000])                        # exact integers
+    u[1000:2000] = np.round(u[1000:2000] * 2) / 2        # half-integers
+    c = np.floor(u).astype(np.int64) + rng.integers(-3, 5, size=n)
+    u64 = u.astype(np.float64)
+    i32 = oracle.table_index(u64, c, 4096, 32)
+    i64 = oracle.table_index(u64, c, 4096, 64)
+    assert np.array_equal(i32, i64)
+    for k in rng.integers(0, n, size=300).tolist() + list(range(0, 2000, 40)):       # exact arithmetic on a sample
+        d = abs(Fraction(float(u[k])) - int(c[k]))
+        assert int(i32[k]) == math.floor(d * 4096 + Fraction(1, 2)), (float(u[k]), int(c[k]))
+    # numpy's own float64 evaluation of the same rule agrees everywhere
+    assert np.array_equal(i64, np.floor(np.abs(u64 - c) * 4096 + 0.5).astype(np.int64))
+    # not a power of two: |index difference| <= 1, on a small fraction of the inputs
+    j32 = oracle.table_index(u64, c, 1000, 32)
+    j64 = oracle.table_index(u64, c, 1000, 64)
+    diff = np.abs(j32 - j64)
+    assert diff.max() <= 1
+    rate = float((diff > 0).mean())
+    assert rate < 2e-3, rate
+    # small |u| (< 1): the subtraction u - c itself rounds in fp32; still at most one sample apart at R = 4096
+    us = rng.uniform(-1.0, 1.0, size=20000).astype(np.float32).astype(np.float64)
+    cs = rng.integers(-3, 4, size=20000)
+    assert np.abs(oracle.table_index(us, cs, 4096, 32) - oracle.table_index(us, cs, 4096, 64)).max() <= 1
 
 
 def test_power_method_vs_dense_eigensolver():
