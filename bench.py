@@ -3,13 +3,18 @@
 Phi^dagger at M = 1e8 on one B200; % of HBM roofline).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 4] [--M m]
+                    [--dtype c64|c128] [--order generated|shuffled] [--scaling weak|strong] [--ubench]
 
 A "step" is one pass of the whole hot path, Phi^dagger Phi (S+Z, F, W G, G^dagger W^dagger,
-F^dagger, Z^dagger S^dagger) over the config's visibility set; for N > 1 every
-rank owns its own M visibilities (the paper's data-parallel scheme) and the step
-ends with the all-reduce of the image (Eq. 38).  value = (visibilities all ranks processed) / time.
-Prints ONE JSON line on rank 0.  `--impl reference` times the CPU oracle (the only reference there
-is: the paper ships no code) on a bounded sample, on the host cores.
+F^dagger, Z^dagger S^dagger) over the config's visibility set.  For N > 1 the paper's
+distributed-image scheme (Algorithm 2): every rank owns its share of the visibilities and a
+replica of the image, and the step ends with the all-reduce of the image (Eq. 38), issued band by band from inside
+purify_normal_dist.  --scaling weak: every rank draws its OWN M visibilities; strong: ONE set of M visibilities is
+cut into equal contiguous sections.  value = (visibilities all ranks processed) / time.
+`--gpus N` without a torchrun environment starts the N ranks itself (torch.distributed.run --standalone).
+Prints ONE JSON line on rank 0.  `--impl reference` times the CPU oracle (the only reference there is: the paper
+ships no code) on a bounded sample, on the host cores.  `--ubench` prints the issue rates of the packed-fp32
+instruction forms the kernels consist of (the measured ALU ceiling of DESIGN.md 5).
 """
 from __future__ import annotations
 
@@ -40,8 +45,13 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--M", type=int, default=0, help="override the number of visibilities (debug)")
-    ap.add_argument("--cpu-sample", type=int, default=4_000_000, help="visibilities in the oracle sample")
+    ap.add_argument("--dtype", default="", choices=["", "c64", "c128"], help="override the config's dtype (config 3: both)")
+    ap.add_argument("--order", default="generated", choices=["generated", "shuffled"],
+                    help="order of the visibilities handed to create (config 3: time-ordered and shuffled)")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"])
+    ap.add_argument("--cpu-sample", type=int, default=4_000_000, help="visibilities in the oracle sample (--impl reference; M > 1e8)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ubench", action="store_true", help="only the packed-fp32 issue-rate probe")
     return ap.parse_args()
 
 
@@ -108,16 +118,15 @@ class ClockSampler:
 
 
 # ----------------------------------------------------------------------------------- oracle timing
-def time_oracle(cfg, x, uv, w, sample: int):
-    """The CPU oracle as it stands on a bounded sample: the K x K stages (pad, FFT, inverse FFT, crop)
-    at full size, the O(M J^2) stages (degrid, grid) on the first `sample` visibilities, extrapolated
-    linearly in M (operator time is linear in M)."""
+def time_oracle(cfg, x, uv, w, sample: int, dtype: str):
+    """The CPU oracle as it stands: the K x K stages (pad, FFT, inverse FFT, crop) at full size, the O(M J^2) stages
+    (degrid, grid) on the first `sample` visibilities (sample = M: the whole set, nothing extrapolated)."""
     import oracle
     ms = min(sample, len(uv))
     uvs = uv[:ms].astype(np.float64)
     ws = w[:ms].astype(np.float64)
     mode = cfg.kernel_mode
-    prec = 32 if cfg.dtype == "c64" else 64
+    prec = 32 if dtype == "c64" else 64
     t0 = time.perf_counter()
     B = oracle.fft2(oracle.pad(x, cfg.J), -1)
     t1 = time.perf_counter()
@@ -135,11 +144,21 @@ def time_oracle(cfg, x, uv, w, sample: int):
 
 def cpu_baseline_entry(cfg, M, res):
     full = res["fixed_s"] + M * res["per_vis_s"]
-    return {"value": M / full, "unit": UNIT, "cores": res["cores"], "kind": "oracle",
-            "sample": (f"oracle/ (fp64 C++, OpenMP): pad+FFT+iFFT+crop at full {cfg.K}x{cfg.K} "
-                       f"({res['fixed_s']:.2f} s) + degrid ({res['degrid_s']:.2f} s) and grid ({res['grid_s']:.2f} s) "
-                       f"on the first {res['sample']} of {M} visibilities, extrapolated linearly in M "
-                       f"to {full:.1f} s per Phi^dagger Phi")}
+    if res["sample"] >= M:
+        what = (f"oracle/ (fp64 C++, OpenMP) timed ONCE AT FULL SIZE: pad+FFT+iFFT+crop at {cfg.K}x{cfg.K} "
+                f"({res['fixed_s']:.2f} s) + degrid ({res['degrid_s']:.2f} s) + grid ({res['grid_s']:.2f} s) over all {M} "
+                f"visibilities = {full:.1f} s per Phi^dagger Phi (nothing extrapolated)")
+    else:
+        what = (f"oracle/ (fp64 C++, OpenMP): pad+FFT+iFFT+crop at full {cfg.K}x{cfg.K} "
+                f"({res['fixed_s']:.2f} s) + degrid ({res['degrid_s']:.2f} s) and grid ({res['grid_s']:.2f} s) "
+                f"on the first {res['sample']} of {M} visibilities, EXTRAPOLATED linearly in M (PAPER.md:608) "
+                f"to {full:.1f} s per Phi^dagger Phi")
+    return {"value": M / full, "unit": UNIT, "cores": res["cores"], "kind": "oracle", "sample": what,
+            "extrapolated": res["sample"] < M}
+
+
+def effective_dtype(cfg, args):
+    return args.dtype or cfg.dtype
 
 
 def run_reference(args):
@@ -148,64 +167,131 @@ def run_reference(args):
         return
     from inputs import synth
     cfg = synth.CONFIGS[args.config]
+    dtype = effective_dtype(cfg, args)
     M = args.M or cfg.M
     ms = min(args.cpu_sample, M)
-    x = synth.make_image(cfg.n, cfg.seed, cfg.dtype)
+    x = synth.make_image(cfg.n, cfg.seed, dtype)
     uv = synth.make_uv(cfg, ms)
     w = synth.make_weights(cfg, ms)
     runs = []
     for i in range(args.warmup + args.steps):
-        r = time_oracle(cfg, x, uv, w, ms)
+        r = time_oracle(cfg, x, uv, w, ms, dtype)
         if i >= args.warmup:
             runs.append(r)
     fixed = statistics.mean(r["fixed_s"] for r in runs)
     per_vis = statistics.mean(r["per_vis_s"] for r in runs)
     full = fixed + M * per_vis
     agg = dict(runs[-1], fixed_s=fixed, per_vis_s=per_vis)
-    value = args.gpus * M / full if args.gpus > 1 else M / full
     line = {"impl": "reference", "metric": METRIC, "value": M / full, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": full * 1e3, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": workload(cfg, M, args.gpus),
+            "scaling": args.scaling, "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload(cfg, M, args.gpus, dtype, args),
             "cpu_baseline": cpu_baseline_entry(cfg, M, agg),
             "e2e": {"value": M / full, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
-    del value
     print(json.dumps(line), flush=True)
 
 
-def alu_roofline(cfg, M, stage_ms):
-    """fp32 FMA work of W G / G^dagger W^dagger per visibility (ANALYTIC mode): the J x J complex-times-real MACs
-    (2 J^2 + 2 J FMA for degridding, 2 J^2 + 2 J + 2 for gridding) plus the paired even/odd Horner chains of the
-    kernel weights, 2 axes x J/2 pairs x (deg + 1) FMA + 6; TABLE mode: the MACs only.  Peak: nominal plain-ALU fp32."""
-    if cfg.dtype != "c64":
+# ----------------------------------------------------------------------------------- ALU ceiling
+FORM_2FFMA, FORM_ROW, FORM_PAIR, FORM_HORNER, FORM_GRID = range(5)
+
+
+def instruction_mix(J, kernel_mode, dtype):
+    """Packed-fp32 instructions of ONE visibility by instruction form (csrc/ubench.cuh), complex64 ANALYTIC:
+    Horner steps of the paired even / odd polynomials of both axes (degree 8 at J = 4, 7 otherwise) + t and t^2;
+    two combinations t O + E per tap pair; the J x J complex-times-real MACs, the J column MACs and the weight."""
+    if dtype != "c64" or kernel_mode == "table":
         return None
-    J = cfg.J
     deg = 8 if J == 4 else 7
-    wts = 0 if cfg.kernel_mode == "table" else 2 * (J // 2) * (deg + 1) + 6
-    fma = {"degrid": 2 * J * J + 2 * J + 2 + wts, "grid": 2 * J * J + 2 * J + 2 + wts}
-    peak = 148 * 128 * 2 * 1.965e9 / 1e12
-    out = {"bound": "alu", "unit": "TFLOP/s", "peak": peak,
-           "peak_source": "nominal: 148 SMs x 128 fp32 lanes x 2 flop x 1.965 GHz (DESIGN.md 5)"}
-    for k, f in fma.items():
-        if stage_ms.get(k):
-            ach = 2.0 * f * M / (stage_ms[k] * 1e-3) / 1e12
-            out[k] = {"fma_per_visibility": f, "achieved": ach, "frac": ach / peak}
+    ne, no = deg // 2 + 1, (deg + 1) // 2
+    horner = (J // 2) * ((ne - 1) + (no - 1)) + 2
+    combine = J
+    return {"degrid": {FORM_HORNER: horner, FORM_PAIR: combine, FORM_ROW: J * J + J + 2},
+            "grid": {FORM_HORNER: horner, FORM_PAIR: combine, FORM_GRID: J * J + J + 1}}
+
+
+def measure_forms(warps_per_sm=16):
+    from paper_1903_04502_b200 import UBENCH_FORMS, ubench_fma
+    out = []
+    for f, name in enumerate(UBENCH_FORMS):
+        cyc, ghz = ubench_fma(f, warps_per_sm)
+        out.append({"form": f, "what": name, "cycles_per_instruction_per_sub_partition": cyc, "sm_ghz_under_this_load": ghz})
     return out
 
 
-def workload(cfg, M, gpus):
+def alu_roofline(cfg, dtype, n_iterations, stage_ms, forms, sm_ghz):
+    """Time the two kernels would need if nothing but their packed-fp32 instructions were issued, each at the rate the
+    probe measured for its form on THIS device (operand-bandwidth bound forms included): iterations (32 slots each,
+    padding included - a padding slot does the full arithmetic) x sum over forms of count x cycles, over 4
+    sub-partitions x SMs at the SM clock seen under the kernels."""
+    mix = instruction_mix(cfg.J, cfg.kernel_mode, dtype)
+    if mix is None or forms is None:
+        return None
+    import torch
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    cyc = {f["form"]: f["cycles_per_instruction_per_sub_partition"] for f in forms}
+    out = {"bound": "alu", "unit": "ms", "peak_measured": forms, "sm_ghz_assumed": sm_ghz,
+           "nominal_fp32_tflops": sms * 128 * 2 * 1.965e9 / 1e12,
+           "note": ("floor_ms: every packed-fp32 instruction at the issue rate bench.py measured for its form "
+                    "(purify_ubench_fma, clock64 cycles); frac = floor_ms / kernel_ms")}
+    for k, m in mix.items():
+        if stage_ms.get(k):
+            cycles = sum(n * cyc[f] for f, n in m.items())
+            floor_ms = n_iterations * cycles / (4 * sms) / (sm_ghz * 1e9) * 1e3
+            out[k] = {"instructions_per_visibility": sum(m.values()), "cycles_per_visibility_slot_warp": cycles,
+                      "floor_ms": floor_ms, "frac": floor_ms / stage_ms[k]}
+    return out
+
+
+def run_ubench(args):
+    import torch
+    assert torch.cuda.is_available(), "--ubench needs a CUDA device"
+    res = {"ubench": "packed fp32 issue rates (csrc/ubench.cuh)", "device": torch.cuda.get_device_name(0),
+           "by_warps_per_sm": {str(w): measure_forms(w) for w in (4, 8, 16, 32)}}
+    print(json.dumps(res), flush=True)
+
+
+def workload(cfg, M, gpus, dtype, args):
+    per_vis = 20 if dtype == "c64" else 40
+    cb = 8 if dtype == "c64" else 16
     return {"workload": f"BASELINE.json configs[{cfg.index - 1}] ({cfg.name}): {cfg.n}x{cfg.n} image, "
-                        f"{cfg.K}x{cfg.K} grid, Kaiser-Bessel J={cfg.J}, M={M} visibilities per GPU, "
-                        f"uv={cfg.uv}, {cfg.dtype}, kernel={cfg.kernel_mode}",
-            "n": cfg.n, "K": cfg.K, "J": cfg.J, "M_per_gpu": M, "M_total": M * gpus, "uv": cfg.uv,
+                        f"{cfg.K}x{cfg.K} grid, Kaiser-Bessel J={cfg.J}, M={M} visibilities "
+                        f"{'per GPU' if args.scaling == 'weak' else 'in total'}, uv={cfg.uv} ({args.order} order), {dtype}, "
+                        f"kernel={cfg.kernel_mode}",
+            "n": cfg.n, "K": cfg.K, "J": cfg.J, "uv": cfg.uv, "order": args.order, "dtype": dtype,
+            "M_per_gpu": M if args.scaling == "weak" else None, "M_total": M * gpus if args.scaling == "weak" else M,
             "kernel_mode": cfg.kernel_mode, "y_order": "native (tile-sorted) inside Phi^dagger Phi",
-            "l2": (f"inputs exceed L2 (no flush needed): every step streams {M * (20 if cfg.dtype == 'c64' else 40) / 1e9:.2f} GB of "
-                   f"visibility data + the {cfg.K * cfg.K * (8 if cfg.dtype == 'c64' else 16) / 1e6:.0f} MB grid"
-                   if M * 20 > 126e6 else "working set fits L2: times are L2-resident, no roofline claim"),
-            "parallelism": f"dp{gpus} over visibilities, all-reduce of the image after Phi^dagger" if gpus > 1 else "single GPU"}
+            "l2": (f"inputs exceed L2 (no flush needed): every step streams {M * per_vis / 1e9:.2f} GB of "
+                   f"visibility data + the {cfg.K * cfg.K * cb / 1e6:.0f} MB grid"
+                   if M * per_vis > 126e6 else "working set fits L2: times are L2-resident, no roofline claim"),
+            "parallelism": (f"dp{gpus} over visibilities ({args.scaling} scaling), all-reduce of the image after Phi^dagger, "
+                            f"issued in bands from purify_normal_dist" if gpus > 1 else "single GPU")}
+
+
+def measured_traffic(cfg, M, dtype, order, kernel):
+    """DRAM bytes of one launch from the ncu capture named in profiles/traffic.json for exactly this workload, or None."""
+    try:
+        tab = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
+        ent = tab.get(f"config{cfg.index}_M{M}_{dtype}_{cfg.kernel_mode}_{order}")
+        if ent:
+            return ent.get(kernel), ent.get("source")
+    except Exception:
+        pass
+    return None, None
 
 
 # ----------------------------------------------------------------------------------- our arm
+def respawn_under_torchrun(args):
+    """`--gpus N` outside a torchrun environment: start the N ranks ourselves, one per GPU."""
+    import torch
+    if torch.cuda.device_count() < args.gpus:
+        raise SystemExit(f"bench.py --gpus {args.gpus}: only {torch.cuda.device_count()} CUDA device(s) visible")
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")              # the communicator / transport lines go to stderr
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--standalone", "--local-addr", "127.0.0.1", "--nnodes=1",
+           f"--nproc-per-node={args.gpus}", os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd, env=env))
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -217,21 +303,34 @@ def run_ours(args):
     rank, local_rank, world = pdist.world()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference for the oracle)")
+    if world != args.gpus:
+        raise SystemExit(f"bench.py --gpus {args.gpus} launched with WORLD_SIZE={world}")
     torch.cuda.set_device(local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
     cfg = synth.CONFIGS[args.config]
+    dtype = effective_dtype(cfg, args)
     M = args.M or cfg.M
-    dt = C64 if cfg.dtype == "c64" else C128
-    cbytes = 8 if cfg.dtype == "c64" else 16
+    dt = C64 if dtype == "c64" else C128
+    cbytes = 8 if dtype == "c64" else 16
     rbytes = cbytes // 2
-    # every rank draws its OWN visibility set (weak scaling): seed offset by rank
-    rcfg = pdist.rank_config(cfg, rank)
+    rd = synth.real_dtype(dtype)
     t_gen = time.perf_counter()
-    x = synth.make_image(cfg.n, cfg.seed, cfg.dtype)
-    uv = synth.make_uv(rcfg, M)
-    w = synth.make_weights(rcfg, M)
+    x = synth.make_image(cfg.n, cfg.seed, dtype)
+    if args.scaling == "weak":                      # every rank draws its OWN visibility set: seed offset by rank
+        rcfg = pdist.rank_config(cfg, rank)
+        uv = synth.make_uv(rcfg, M).astype(rd, copy=False)
+        w = synth.make_weights(rcfg, M).astype(rd, copy=False)
+        M_rank, M_job = M, M * world
+    else:                                           # ONE set, cut into equal contiguous sections
+        lo, hi = pdist.shard_bounds(M, rank, world)
+        uv = np.ascontiguousarray(synth.make_uv(cfg, M)[lo:hi]).astype(rd, copy=False)
+        w = np.ascontiguousarray(synth.make_weights(cfg, M)[lo:hi]).astype(rd, copy=False)
+        M_rank, M_job = hi - lo, M
+    if args.order == "shuffled":
+        order = synth.shuffle_order(len(uv), cfg.seed + rank)
+        uv, w = np.ascontiguousarray(uv[order]), np.ascontiguousarray(w[order])
     t_gen = time.perf_counter() - t_gen
 
     x_pin = torch.from_numpy(x).pin_memory()
@@ -241,15 +340,18 @@ def run_ours(args):
     t_create = time.perf_counter()
     op = PurifyOp(cfg.n, cfg.J, torch.from_numpy(uv).cuda(), torch.from_numpy(w).cuda(), dtype=dt,
                   kernel_mode=TABLE if cfg.kernel_mode == "table" else ANALYTIC,
-                  table_samples_per_unit=cfg.table_R if cfg.kernel_mode == "table" else 0, time_stages=True)
+                  table_samples_per_unit=cfg.table_R if cfg.kernel_mode == "table" else 0)
     torch.cuda.synchronize()
     t_create = time.perf_counter() - t_create
     info = op.info()
     torch.cuda.empty_cache()
 
-    def step():
-        op.normal(x_dev, out_dev)
-        pdist.allreduce_image(out_dev)                          # Eq. (38): sum of the per-rank dirty images
+    if world > 1:
+        def step():                                 # Eq. (38): the bands of the image are summed over the ranks as they are cropped
+            op.normal_dist(x_dev, out_dev, allreduce=lambda band: dist.all_reduce(band, op=dist.ReduceOp.SUM))
+    else:
+        def step():
+            op.normal(x_dev, out_dev)
 
     def barrier():
         if world > 1:
@@ -278,12 +380,14 @@ def run_ours(args):
     ms_total = pdist.max_over_ranks(ms_total, device="cuda")
     ms_step = ms_total / args.steps
 
-    # ---- per-stage breakdown (separate pass; each step followed by a sync to read the stage events)
+    # ---- per-stage breakdown (separate pass with the stage events switched on: launches issued one by one, no graph)
+    op.set_time_stages(True)
     stages = {}
     for _ in range(args.steps):
         op.normal(x_dev, out_dev)
         for k, v in op.stage_times_ms().items():
             stages.setdefault(k, []).append(v)
+    op.set_time_stages(False)
     stage_ms = {k: statistics.mean(v) for k, v in stages.items()}
     clocks = sampler.stop() if sampler else None
 
@@ -306,6 +410,12 @@ def run_ours(args):
     y_call = op.permute_from_native(y_dev)
     ms_phi_caller = timed(lambda: op.degrid(x_dev, y_call, native=False), reps)
     ms_phit_caller = timed(lambda: op.grid(y_call, out_dev, native=False), reps)
+    op.set_time_stages(True)
+    op.degrid(x_dev, y_call, native=False)
+    ms_permute_out = op.stage_times_ms()["permute"]
+    op.grid(y_call, out_dev, native=False)
+    ms_permute_in = op.stage_times_ms()["permute"]
+    op.set_time_stages(False)
     del y_call
 
     # ---- f2: power method on Phi^dagger Phi, 10 iterations from the all-ones vector
@@ -326,73 +436,91 @@ def run_ours(args):
                  "note": "purify_admm_fidelity_step: v = Phi x, l2-ball projection, dual update, Phi^dagger (v - r + s)"}
     del y_obs, s_dual
 
-    # ---- end to end through the C ABI with HOST buffers (H2D of x, D2H of the result inside)
-    op.normal_host(x_pin, out_pin)
+    # ---- end to end with HOST buffers: H2D of x and D2H of the result inside the timed region.  One GPU: the C-ABI call
+    # purify_normal_host.  N GPUs: pinned copies around the distributed step (the all-reduce included).
+    def e2e_step():
+        if world == 1:
+            op.normal_host(x_pin, out_pin)
+        else:
+            x_dev.copy_(x_pin, non_blocking=True)
+            step()
+            out_pin.copy_(out_dev, non_blocking=True)
+            torch.cuda.synchronize()
+    e2e_step()
     barrier()
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        op.normal_host(x_pin, out_pin)
-        if world > 1:
-            pass    # the host-buffer path is single-GPU; the image all-reduce is in the device arm
+        e2e_step()
     torch.cuda.synchronize()
     e2e_s = (time.perf_counter() - t0) / args.steps
     e2e_s = pdist.max_over_ranks(e2e_s, device="cuda")
+
+    forms = measure_forms(16) if (rank == 0 and dtype == "c64") else None
 
     if rank == 0:
         peak, peak_src = measured_peak()
         K = cfg.K
         per_vis = 2 * rbytes + rbytes + cbytes                       # uv + w + y  (20 B / 40 B)
-        alg_bytes = M * per_vis + K * K * cbytes                      # + the grid, once
+        alg_bytes = M_rank * per_vis + K * K * cbytes                 # + the grid, once
         dom = "degrid" if stage_ms.get("degrid", 0) >= stage_ms.get("grid", 0) else "grid"
         dom_ms = stage_ms[dom]
         achieved = alg_bytes / (dom_ms * 1e-3) / 1e9
-        traffic = None
-        try:    # measured DRAM traffic of the dominant kernel (ncu capture under profiles/), same workload only
-            tr = json.load(open(os.path.join(ROOT, "profiles", "r1f_traffic.json.txt")))
-            traffic = tr.get(f"config{cfg.index}_M{M}", {}).get(dom)
-        except Exception:
-            traffic = None
         kname = f"{dom}_x_kernel" if info["layout"] == 1 else f"{dom}_kernel"
+        traffic, traffic_src = measured_traffic(cfg, M_rank, dtype, args.order, dom)
+        # bytes the kernel is MADE to stream by the layout: records (12 B or 24 B per slot) + y per slot + lane words and
+        # batch headers + the box of every work item (degridding reads it, gridding reduces it into the grid)
+        box = (32 + cfg.J) * (16 + cfg.J - 1) * cbytes
+        streamed = (info["M_native"] * (3 * rbytes + cbytes) + info["n_batches"] * 136 + info["n_items"] * (32 + box)
+                    if info["layout"] == 1 else None)
+        sm_ghz = (clocks or {}).get("sm_mhz") or 1965.0
         line = {
-            "metric": METRIC, "value": world * M / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world,
+            "metric": METRIC, "value": M_job / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step,
             "ms_per_step_stats": {"mean": statistics.mean(per_step), "std": statistics.pstdev(per_step), "min": min(per_step),
                                   "max": max(per_step), "note": "rank 0, per-step CUDA events inside the timed region"},
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32" if cfg.dtype == "c64" else "f64", "data": "synthetic",
-            "config": workload(cfg, M, world),
-            "e2e": {"value": world * M / e2e_s, "unit": UNIT, "ms_per_step": e2e_s * 1e3,
+            "higher_is_better": True, "scaling": args.scaling, "vs_baseline": None,
+            "dtype": "f32" if dtype == "c64" else "f64", "data": "synthetic",
+            "config": workload(cfg, M, world, dtype, args),
+            "e2e": {"value": M_job / e2e_s, "unit": UNIT, "ms_per_step": e2e_s * 1e3,
                     "h2d_bytes_per_step": int(x_pin.numel() * cbytes), "d2h_bytes_per_step": int(out_pin.numel() * cbytes),
-                    "api": "purify_normal_host (pinned host x in, host x out)"},
+                    "api": ("purify_normal_host (pinned host x in, host x out)" if world == 1 else
+                            "pinned H2D of x + purify_normal_dist (all-reduce inside) + D2H of the image, per rank")},
             "gpu_launches": launches,
             "roofline": {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "peak_source": peak_src, "traffic": traffic,
-                         "note": "HBM fraction of the ALGORITHMIC bytes; the kernel itself is fp32-FMA bound (profiles/r1f_summary.md)",
+                         "frac": achieved / peak, "peak_source": peak_src,
+                         "traffic": traffic, "traffic_source": traffic_src,
+                         "traffic_over_algorithmic": (traffic / alg_bytes) if traffic else None,
+                         "streamed_bytes_by_layout": streamed,
+                         "streamed_over_algorithmic": (streamed / alg_bytes) if streamed else None,
+                         "note": ("HBM fraction of the ALGORITHMIC bytes; the kernels themselves are bound by the issue rate of "
+                                  "their packed-fp32 instructions (register-operand bandwidth): roofline_alu"),
                          "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": dom_ms,
                          "frac_of_8TBs": achieved / 8000.0,
                          "other_kernel": {k: {"ms": stage_ms[k], "achieved": alg_bytes / (stage_ms[k] * 1e-3) / 1e9,
                                               "frac": alg_bytes / (stage_ms[k] * 1e-3) / 1e9 / peak}
                                           for k in ("degrid", "grid") if k != dom}},
-            # the same kernels against the plain-ALU fp32 ceiling (they are FMA-bound, not HBM-bound):
-            # algorithmic flops = M x (4 J^2 + 4 J complex-times-real MAC flops + weight evaluation), peak = 148 SMs x
-            # 128 fp32 lanes x 2 flop x 1.965 GHz
-            "roofline_alu": alu_roofline(cfg, M, stage_ms),
+            "roofline_alu": alu_roofline(cfg, dtype, info["M_native"] / 32, stage_ms, forms, sm_ghz / 1e3),
             "stage_ms": stage_ms,
-            "operators": {"phi_ms": ms_phi, "phi_vis_per_s": M / (ms_phi * 1e-3),
-                          "phi_dagger_ms": ms_phit, "phi_dagger_vis_per_s": M / (ms_phit * 1e-3),
-                          "phi_caller_order_ms": ms_phi_caller, "phi_dagger_caller_order_ms": ms_phit_caller},
+            "stage_ms_sum_vs_step": {"sum": sum(stage_ms.values()), "step": ms_step,
+                                     "note": "stages timed with the launches issued one by one; the step replays a CUDA graph"},
+            "operators": {"phi_ms": ms_phi, "phi_vis_per_s": M_rank / (ms_phi * 1e-3),
+                          "phi_dagger_ms": ms_phit, "phi_dagger_vis_per_s": M_rank / (ms_phit * 1e-3),
+                          "phi_caller_order_ms": ms_phi_caller, "phi_dagger_caller_order_ms": ms_phit_caller,
+                          "permute_from_native_ms": ms_permute_out, "permute_to_native_ms": ms_permute_in},
             "operator_norm": norm_info,
             "admm_fidelity_step": admm_info,
             "clocks": clocks,
             "setup": {"generate_s": t_gen, "create_s": t_create, "n_items": info["n_items"],
                       "n_tiles_nonempty": info["n_tiles_nonempty"], "max_tile_count": info["max_tile_count"],
                       "device_bytes": info["device_bytes"], "M_native": info["M_native"],
-                      "padding_ratio": info["M_native"] / max(M, 1), "n_batches": info["n_batches"]},
+                      "padding_ratio": info["M_native"] / max(M_rank, 1), "n_batches": info["n_batches"]},
         }
         if world == 1 and not args.no_cpu_baseline:
-            ms = min(args.cpu_sample, M)
-            res = time_oracle(cfg, x, uv[:ms], w[:ms], ms)
-            line["cpu_baseline"] = cpu_baseline_entry(cfg, M, res)
+            # the oracle timed ONCE at full size where that takes about half a minute (M <= 1e8); a 4e6 sample beyond
+            ms = M_rank if M_rank <= 100_000_000 else min(args.cpu_sample, M_rank)
+            res = time_oracle(cfg, x, uv[:ms], w[:ms], ms, dtype)
+            line["cpu_baseline"] = cpu_baseline_entry(cfg, M_rank, res)
+            line["vs_cpu_baseline"] = line["value"] / line["cpu_baseline"]["value"]
         print(json.dumps(line), flush=True)
     op.close()
     if world > 1:
@@ -403,7 +531,11 @@ def main():
     args = parse()
     if args.impl == "reference":
         run_reference(args)
+    elif args.ubench:
+        run_ubench(args)
     else:
+        if args.gpus > 1 and "RANK" not in os.environ:
+            respawn_under_torchrun(args)
         run_ours(args)
 
 

@@ -1,7 +1,10 @@
 """Data-parallel plumbing of the operator over visibilities (Eq. 37-38): every rank
 holds a replica of the image and its own visibilities; Phi needs no exchange, Phi^dagger ends with an
-all-reduce(sum) of the n x n image.  torch.distributed only (NCCL on GPUs, gloo in the CPU tests);
-no method arithmetic here and no import of oracle/ or of the CUDA library."""
+all-reduce(sum) of the n x n image.  On the CUDA path the exchange is issued from INSIDE the operator
+(purify_grid_dist / purify_normal_dist hand the image to an all-reduce callback band by band, overlapped with the
+crop - PurifyOp.normal_dist(x, out, allreduce=lambda band: dist.all_reduce(band))); this module holds what is left
+for the host: the rank environment, who owns which visibilities, the timing rule.  torch.distributed only (NCCL on
+GPUs, gloo in the CPU tests); no method arithmetic here and no import of oracle/ or of the CUDA library."""
 from __future__ import annotations
 
 import dataclasses
