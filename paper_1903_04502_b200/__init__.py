@@ -6,3 +6,4 @@
 there is no CPU fallback.  The seeded input generators live outside the package, in `inputs/`.
 """
 from .op import ANALYTIC, C64, C128, TABLE, UBENCH_FORMS, PurifyError, PurifyOp, load_library, ubench_fma  # noqa: F401
+from .wavelet import Wavelet  # noqa: F401,E402

@@ -9,8 +9,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpurify_op.so")
-SOURCES = ["purify_op.cu"]
-DEPS = ["purify_op.cu", "kernels.cuh", "degrid.cuh", "grid.cuh", "batched.cuh", "kb_host.hpp", "ubench.cuh",
+SOURCES = ["purify_op.cu", "wavelet.cu"]
+DEPS = ["purify_op.cu", "kernels.cuh", "degrid.cuh", "grid.cuh", "batched.cuh", "kb_host.hpp", "ubench.cuh", "wavelet.cu", os.path.join("..", "..", "include", "purify_wavelet.h"),
         os.path.join("..", "..", "include", "purify_op.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared"]

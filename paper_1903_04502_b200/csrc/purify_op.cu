@@ -69,6 +69,16 @@ constexpr int deg_c128(int J) { return J == 4 ? 17 : (J == 6 ? 16 : 15); }
 
 }  // namespace
 
+namespace pkerr {
+int set(int status, const char* fmt, ...) {          // the detail string is shared with wavelet.cu (same library)
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return status;
+}
+}  // namespace pkerr
+
 struct purify_op {
     int n = 0, K = 0, J = 0, dtype = 0, mode = 0, table_R = 0, chunk = 4096, time_stages = 0;
     long long M = 0;

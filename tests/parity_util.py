@@ -39,9 +39,13 @@ def errors(a, ref):
     return (num / den) ** 0.5, dmax / rmax
 
 
-def compare(label, a, ref, tol, l2_factor=1.0, **ctx):
-    """Assert both bounds; returns the rel-L2.  `l2_factor` (a multiple of tol) is 1 everywhere today."""
+def compare(label, a, ref, tol, l2_factor=1.0, scale=None, **ctx):
+    """Assert both bounds; returns the rel-L2.  `l2_factor` (a multiple of tol) is 1 everywhere today.
+    `scale`: magnitude the element-wise deviation is measured against when max|ref| is not the natural one (a clipped
+    output whose inputs are much larger than its values)."""
     l2, linf = errors(a, ref)
+    if scale is not None:
+        linf = linf * float(np.abs(np.asarray(ref)).max()) / float(scale)
     if os.path.isdir(_LOG):
         with open(os.path.join(_LOG, "parity_r2.jsonl"), "a") as fh:
             fh.write(json.dumps(dict(label=label, rel_l2=l2, max_abs_over_max_ref=linf, tol=tol, l2_factor=l2_factor,

@@ -9,8 +9,8 @@ import pytest
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def header_symbols():
-    src = open(os.path.join(ROOT, "include", "purify_op.h")).read()
+def header_symbols(name="purify_op.h"):
+    src = open(os.path.join(ROOT, "include", name)).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(purify_[a-z_0-9]+)\s*\(", src)))
 
@@ -25,6 +25,11 @@ def test_library_builds_and_exports_every_declared_symbol():
     for name in declared:
         assert hasattr(lib, name), f"{name} declared in purify_op.h but not exported"
     assert sorted(op.SYMBOLS) == declared
+    from paper_1903_04502_b200 import wavelet
+    wdeclared = [s for s in header_symbols("purify_wavelet.h") if s not in ("purify_last_error",)]
+    assert sorted(wavelet.SYMBOLS) == wdeclared and len(wdeclared) == 7
+    for name in wdeclared:
+        assert hasattr(lib, name), f"{name} declared in purify_wavelet.h but not exported"
     L = op.load_library()
     assert L.purify_version() >= 100
     assert L.purify_strerror(-7).decode().startswith("no CUDA device")
