@@ -436,6 +436,30 @@ def run_ours(args):
                  "note": "purify_admm_fidelity_step: v = Phi x, l2-ball projection, dual update, Phi^dagger (v - r + s)"}
     del y_obs, s_dual
 
+    # ---- f4: the sparsity side of the iteration (Algorithm 1 line 7 with ONE DUALFB pass, as the paper's Fig. 3 times it):
+    # Psi^dagger, Psi and the pass itself on the n x n image (Dirac + Daubechies 1-8, 3 levels)
+    from paper_1903_04502_b200 import Wavelet
+    wl = Wavelet(cfg.n, 3, dt)
+    alpha = wl.adjoint(x_dev)
+    d_dual = torch.zeros_like(alpha)
+    zbar = wl.project_positive(x_dev)
+    ms_psit = timed(lambda: wl.adjoint(x_dev, alpha), reps)
+    ms_psi = timed(lambda: wl.forward(alpha, out_dev), reps)
+    ms_dualfb = timed(lambda: wl.dualfb_step(x_dev, zbar, d_dual, 1e-3, 9.0, zbar_out=out_dev), reps)
+    nn_bytes = cfg.n * cfg.n * cbytes
+    peak_w, _ = measured_peak()
+    wavelet_info = {
+        "psi_dagger_ms": ms_psit, "psi_ms": ms_psi, "dualfb_pass_ms": ms_dualfb,
+        "algorithmic_bytes": {"psi_dagger": 10 * nn_bytes, "psi": 10 * nn_bytes, "dualfb_pass": (1 + 9 + 9 + 9 + 1 + 1) * nn_bytes},
+        "hbm_frac": {"psi_dagger": 10 * nn_bytes / (ms_psit * 1e-3) / 1e9 / peak_w, "psi": 10 * nn_bytes / (ms_psi * 1e-3) / 1e9 / peak_w,
+                     "dualfb_pass": 30 * nn_bytes / (ms_dualfb * 1e-3) / 1e9 / peak_w},
+        "note": ("algorithmic bytes: image in, 9 coefficient sets out (Psi^dagger) and the reverse (Psi); the DUALFB pass reads zbar, "
+                 "reads and writes d (9 sets), reads z, writes zbar, and must hold Psi^dagger zbar once (9 sets); the kernels "
+                 "make two passes per level through a scratch array, i.e. move about 2.5x that")}
+    admm_iteration_ms = ms_admm + ms_dualfb
+    del alpha, d_dual, zbar
+    wl.close()
+
     # ---- end to end with HOST buffers: H2D of x and D2H of the result inside the timed region.  One GPU: the C-ABI call
     # purify_normal_host.  N GPUs: pinned copies around the distributed step (the all-reduce included).
     def e2e_step():
@@ -509,6 +533,9 @@ def run_ours(args):
                           "permute_from_native_ms": ms_permute_out, "permute_to_native_ms": ms_permute_in},
             "operator_norm": norm_info,
             "admm_fidelity_step": admm_info,
+            "sparsity_prox": wavelet_info,
+            "admm_iteration": {"ms": admm_iteration_ms,
+                               "note": "Algorithm 1 lines 3-7 with one DUALFB pass: purify_admm_fidelity_step + purify_dualfb_step"},
             "clocks": clocks,
             "setup": {"generate_s": t_gen, "create_s": t_create, "n_items": info["n_items"],
                       "n_tiles_nonempty": info["n_tiles_nonempty"], "max_tile_count": info["max_tile_count"],

@@ -105,6 +105,9 @@ grid_kernel(const OpParams<R> p, const typename Cplx<R>::type* __restrict__ y) {
                     t0.x += a0r; t0.y += a0i; t1.x += a1r; t1.y += a1i;
                     d[0] = t0; d[1] = t1;
                 }
+                // (the branch is warp-uniform: `newrun` is a ballot.)  The next run's flush may touch, from ANOTHER lane,
+                // an address this flush has just written: order the two read-modify-write rounds.
+                __syncwarp();
                 a0r = a0i = a1r = a1i = (R)0;
                 cur = __shfl_sync(0xffffffffu, off, kk);
             }

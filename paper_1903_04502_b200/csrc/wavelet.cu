@@ -30,8 +30,9 @@ template <> struct C2T<double> { typedef double2 type; };
 
 struct Filters { int len[NB]; };                          // taps live in device memory: filt[(b * 2 + {0: h, 1: g}) * LMAX + m]
 
-__device__ __forceinline__ int wrap_nonneg(int i, int m) { return i % m; }
-__device__ __forceinline__ int wrap_any(int i, int m) { int r = i % m; return r < 0 ? r + m : r; }
+// periodic index: i is at most a filter length outside [0, m) (no integer division in the tap loops)
+__device__ __forceinline__ int wrap_nonneg(int i, int m) { while (i >= m) i -= m; return i; }
+__device__ __forceinline__ int wrap_any(int i, int m) { while (i < 0) i += m; while (i >= m) i -= m; return i; }
 
 // ---- analysis along x: rows r < m of src (m x m block, pitch `pitch`, one array per basis or one shared array when
 // src_stride == 0) -> tmp[b][r][0..m/2) (low) and [m/2..m) (high)

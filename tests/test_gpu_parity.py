@@ -445,3 +445,76 @@ def test_ubench_fma_forms():
     assert 1.9 <= rates[3] <= 2.2, rates                 # Horner form: pipe-bound
     assert rates[1] >= rates[3] * 1.05, rates            # row-pass form: operand-bound
     assert rates[4] <= rates[1], rates                   # gridding form is the cheaper of the two MAC forms
+
+
+def test_canaries_around_every_output_buffer():
+    """compute-sanitizer is closed on this pool (profiles/r2_sanitizer.md), so out-of-bounds writes are looked for
+    directly: every output of the C ABI is a slice in the MIDDLE of a larger allocation whose flanks hold a canary
+    pattern; after the call the flanks must be untouched.  Sizes chosen ragged (M and M_native not multiples of 32 x
+    the chunk sizes, K not a power of two) so that the last chunk / item / batch / band of every kernel is partial."""
+    from paper_1903_04502_b200 import C64, C128, PurifyOp
+    GUARD = 4096
+
+    def guarded(count, dtype):
+        buf = torch.full((count + 2 * GUARD,), complex(7.25, -3.5), dtype=dtype, device="cuda")
+        return buf, buf[GUARD:GUARD + count]
+
+    def intact(buf, count):
+        return bool((buf[:GUARD] == complex(7.25, -3.5)).all()) and bool((buf[GUARD + count:] == complex(7.25, -3.5)).all())
+
+    rng = synth.rng_for(31337, synth.STREAM_UV)
+    for dtype, dt, cdt in (("c64", C64, torch.complex64), ("c128", C128, torch.complex128)):
+        for n, J, M in ((50, 6, 7001), (34, 4, 333), (64, 8, 5003)):
+            K = 2 * n
+            uv = np.concatenate([rng.uniform(-K / 2, K / 2, size=(M - 300, 2)), 3.0 + rng.uniform(0, 1, size=(300, 2))])
+            uv = uv.astype(synth.real_dtype(dtype))
+            w = rng.uniform(0.5, 1.5, size=M).astype(synth.real_dtype(dtype))
+            op = PurifyOp(n, J, dev(uv), dev(w), dtype=dt)
+            x = dev(synth.random_complex((n, n), seed=1, dtype=dtype))
+            by, y = guarded(M, cdt)
+            bn, yn = guarded(op.M_native, cdt)
+            bx, xo = guarded(n * n, cdt)
+            xo2 = xo.view(n, n)
+            op.degrid(x, y)
+            op.degrid(x, yn, native=True)
+            op.grid(y, xo2)
+            op.grid(yn, xo2, native=True)
+            op.normal(x, xo2)
+            op.normal(x, xo2)
+            op.permute_to_native(y, yn)
+            op.permute_from_native(yn, y)
+            bs, s = guarded(op.M_native, cdt)
+            s.zero_()
+            op.admm_fidelity_step(x, yn, s, 0.5, 0.9, xo2)
+            op.normal_dist(x, xo2, allreduce=lambda band: None, bands=7)
+            torch.cuda.synchronize()
+            assert intact(by, M) and intact(bn, op.M_native) and intact(bx, n * n) and intact(bs, op.M_native), (dtype, n, J, M)
+            op.close()
+
+
+def test_gridding_repeatable_under_stress_on_hot_cells():
+    """The accumulator flush of the gridding kernel is the one place where lanes of a warp write overlapping
+    shared-memory footprints; the steps are ordered by __syncwarp() (batched.cuh).  200 repetitions on the hot-cell
+    input (flagged and unflagged batches, several items per band): every repetition within the tolerance of the
+    oracle, and all repetitions within rounding of one another (a lost update would be an O(1) difference in a cell)."""
+    rng = synth.rng_for(4242, synth.STREAM_UV)
+    n, J = 64, 6
+    K = 2 * n
+    counts = [700, 333, 257, 256, 129, 128, 127, 65, 64, 63]
+    hot = rng.integers(-20, 20, size=(len(counts), 2)).astype(np.float64)
+    parts = [h + rng.uniform(0.0, 1.0, size=(c, 2)) for h, c in zip(hot, counts)]
+    parts.append(rng.uniform(-K / 2, K / 2, size=(6000, 2)))
+    uv = np.concatenate(parts).astype(np.float32)
+    w = rng.uniform(0.5, 1.5, size=len(uv)).astype(np.float32)
+    yv = synth.random_complex((len(uv),), seed=5, dtype="c64")
+    op = make_op(n, J, uv, w, "c64")
+    ref = oracle.grid_to_grid(yv, uv, w, K, J, idx_prec=32)
+    yd = dev(yv)
+    first = op.stage_gridded(yd)
+    compare("stress: gridded", host(first), ref, 1e-5, n=n, J=J, M=len(uv), dtype="c64")
+    scale = float(first.abs().max())
+    worst = 0.0
+    for _ in range(200):
+        worst = max(worst, float((op.stage_gridded(yd) - first).abs().max()) / scale)
+    assert worst <= 2e-6, worst                              # reduction order varies (atomics at L2): rounding only
+    op.close()
