@@ -45,6 +45,7 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--M", type=int, default=0, help="override the number of visibilities (debug)")
+    ap.add_argument("--J", type=int, default=0, help="override the kernel support (4, 6, 8): e.g. the complex128 J = 8 kernels on config 2")
     ap.add_argument("--dtype", default="", choices=["", "c64", "c128"], help="override the config's dtype (config 3: both)")
     ap.add_argument("--order", default="generated", choices=["generated", "shuffled"],
                     help="order of the visibilities handed to create (config 3: time-ordered and shuffled)")
@@ -161,12 +162,19 @@ def effective_dtype(cfg, args):
     return args.dtype or cfg.dtype
 
 
+def effective_config(args):
+    import dataclasses
+    from inputs import synth
+    cfg = synth.CONFIGS[args.config]
+    return dataclasses.replace(cfg, J=args.J) if args.J else cfg
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     from inputs import synth
-    cfg = synth.CONFIGS[args.config]
+    cfg = effective_config(args)
     dtype = effective_dtype(cfg, args)
     M = args.M or cfg.M
     ms = min(args.cpu_sample, M)
@@ -309,7 +317,7 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
-    cfg = synth.CONFIGS[args.config]
+    cfg = effective_config(args)
     dtype = effective_dtype(cfg, args)
     M = args.M or cfg.M
     dt = C64 if dtype == "c64" else C128

@@ -34,135 +34,210 @@ struct Filters { int len[NB]; };                          // taps live in device
 __device__ __forceinline__ int wrap_nonneg(int i, int m) { while (i >= m) i -= m; return i; }
 __device__ __forceinline__ int wrap_any(int i, int m) { while (i < 0) i += m; while (i >= m) i -= m; return i; }
 
-// ---- analysis along x: rows r < m of src (m x m block, pitch `pitch`, one array per basis or one shared array when
-// src_stride == 0) -> tmp[b][r][0..m/2) (low) and [m/2..m) (high)
+// The per-level kernels below are templated on the filter length L (a switch on the basis picks the instantiation),
+// so that the tap loops unroll and every thread produces several outputs from one sliding window of inputs:
+// KPT low / high pairs (analysis) or 2 KPT samples (synthesis) per thread - about (2 KPT + L) loads instead of KPT L.
+constexpr int KPT = 4;
+
+#define WL_SWITCH_L(b, CALL)                    \
+    switch (b) {                                \
+        case 0: { constexpr int L = 2; CALL; } break;   \
+        case 1: { constexpr int L = 4; CALL; } break;   \
+        case 2: { constexpr int L = 6; CALL; } break;   \
+        case 3: { constexpr int L = 8; CALL; } break;   \
+        case 4: { constexpr int L = 10; CALL; } break;  \
+        case 5: { constexpr int L = 12; CALL; } break;  \
+        case 6: { constexpr int L = 14; CALL; } break;  \
+        default: { constexpr int L = 16; CALL; } break; \
+    }
+
+// ---- the analysis pass along x goes through shared memory: a CTA of 128 threads takes ROW_SPAN outputs of one row,
+// stages the inputs they need with coalesced loads, split into even and odd samples so that the stride-2 reads of
+// neighbouring outputs become unit-stride, and every thread then produces outputs 128 apart: coalesced stores.
+constexpr int ROW_SPAN = 512;           // low / high pairs per CTA
+
+template <typename R, int L>
+__device__ __forceinline__ void row_fwd_body(const typename C2T<R>::type* __restrict__ s, typename C2T<R>::type* __restrict__ t,
+                                             int m, int kb, const R* __restrict__ h, const R* __restrict__ g,
+                                             typename C2T<R>::type* ev, typename C2T<R>::type* od) {
+    typedef typename C2T<R>::type C;
+    const int mh = m >> 1, cnt = min(ROW_SPAN, mh - kb), span = 2 * cnt + L - 2;
+    for (int e = threadIdx.x; e < span; e += 128) {
+        const C v = s[wrap_nonneg(2 * kb + e, m)];
+        if (e & 1) od[e >> 1] = v; else ev[e >> 1] = v;
+    }
+    __syncthreads();
+    for (int q = threadIdx.x; q < cnt; q += 128) {
+        R lx = 0, ly = 0, hx = 0, hy = 0;
+#pragma unroll
+        for (int i = 0; i < L; ++i) {
+            const C v = (i & 1) ? od[q + (i >> 1)] : ev[q + (i >> 1)];
+            lx += h[i] * v.x; ly += h[i] * v.y; hx += g[i] * v.x; hy += g[i] * v.y;
+        }
+        C lo; lo.x = lx; lo.y = ly;
+        C hi; hi.x = hx; hi.y = hy;
+        t[kb + q] = lo;
+        t[mh + kb + q] = hi;
+    }
+}
+
 template <typename R>
 __global__ void __launch_bounds__(128) wl_row_fwd(const typename C2T<R>::type* __restrict__ src, long long src_stride, int pitch,
                                                   typename C2T<R>::type* __restrict__ tmp, long long tmp_stride, int n, int m,
-                                                  const R* __restrict__ filt, Filters F) {
+                                                  const R* __restrict__ filt) {
     typedef typename C2T<R>::type C;
-    const int k = blockIdx.x * blockDim.x + threadIdx.x, r = blockIdx.y, b = blockIdx.z, mh = m >> 1;
-    if (k >= mh) return;
+    __shared__ C ev[ROW_SPAN + LMAX / 2], od[ROW_SPAN + LMAX / 2];
+    const int kb = blockIdx.x * ROW_SPAN, r = blockIdx.y, b = blockIdx.z;
     const C* s = src + (long long)b * src_stride + (long long)r * pitch;
+    C* t = tmp + (long long)b * tmp_stride + (long long)r * n;
     const R* h = filt + (b * 2) * LMAX;
     const R* g = h + LMAX;
-    R lx = 0, ly = 0, hx = 0, hy = 0;
-    const int L = F.len[b];
-    for (int i = 0; i < L; ++i) {
-        const C v = s[wrap_nonneg(2 * k + i, m)];
-        const R hi_ = g[i], lo_ = h[i];
-        lx += lo_ * v.x; ly += lo_ * v.y; hx += hi_ * v.x; hy += hi_ * v.y;
-    }
-    C* t = tmp + (long long)b * tmp_stride + (long long)r * n;
-    C lo; lo.x = lx; lo.y = ly;
-    C hi; hi.x = hx; hi.y = hy;
-    t[k] = lo;
-    t[mh + k] = hi;
+    WL_SWITCH_L(b, (row_fwd_body<R, L>(s, t, m, kb, h, g, ev, od)))
 }
 
-// ---- analysis along y: tmp[b] (m x m block) -> dst[b] top-left m x m block (rows [0, m/2) low, [m/2, m) high)
+// ---- analysis along y: tmp[b] (m x m block) -> dst[b] top-left m x m block (rows [0, m/2) low, [m/2, m) high).
+// Thread = one column, KPT consecutive output rows; loads coalesced across the columns.
+template <typename R, int L>
+__device__ __forceinline__ void col_fwd_body(const typename C2T<R>::type* __restrict__ t, typename C2T<R>::type* __restrict__ d,
+                                             int n, int m, int k0, const R* __restrict__ h, const R* __restrict__ g) {
+    typedef typename C2T<R>::type C;
+    const int mh = m >> 1;
+    R lx[KPT], ly[KPT], hx[KPT], hy[KPT];
+#pragma unroll
+    for (int q = 0; q < KPT; ++q) lx[q] = ly[q] = hx[q] = hy[q] = (R)0;
+    int idx = wrap_nonneg(2 * k0, m);
+#pragma unroll
+    for (int r = 0; r < 2 * KPT + L - 2; ++r) {
+        const C v = t[(long long)idx * n];
+        if (++idx == m) idx = 0;
+#pragma unroll
+        for (int q = 0; q < KPT; ++q) {
+            const int i = r - 2 * q;
+            if (i >= 0 && i < L) { lx[q] += h[i] * v.x; ly[q] += h[i] * v.y; hx[q] += g[i] * v.x; hy[q] += g[i] * v.y; }
+        }
+    }
+#pragma unroll
+    for (int q = 0; q < KPT; ++q)
+        if (k0 + q < mh) {
+            C lo; lo.x = lx[q]; lo.y = ly[q];
+            C hi; hi.x = hx[q]; hi.y = hy[q];
+            d[(long long)(k0 + q) * n] = lo;
+            d[(long long)(mh + k0 + q) * n] = hi;
+        }
+}
+
 template <typename R>
 __global__ void __launch_bounds__(128) wl_col_fwd(const typename C2T<R>::type* __restrict__ tmp, long long tmp_stride,
                                                   typename C2T<R>::type* __restrict__ dst, long long dst_stride, int n, int m,
-                                                  const R* __restrict__ filt, Filters F) {
-    typedef typename C2T<R>::type C;
-    const int c = blockIdx.x * blockDim.x + threadIdx.x, k = blockIdx.y, b = blockIdx.z, mh = m >> 1;
+                                                  const R* __restrict__ filt) {
+    const int c = blockIdx.x * blockDim.x + threadIdx.x, k0 = blockIdx.y * KPT, b = blockIdx.z;
     if (c >= m) return;
-    const C* t = tmp + (long long)b * tmp_stride + c;
+    const auto* t = tmp + (long long)b * tmp_stride + c;
+    auto* d = dst + (long long)b * dst_stride + c;
     const R* h = filt + (b * 2) * LMAX;
     const R* g = h + LMAX;
-    R lx = 0, ly = 0, hx = 0, hy = 0;
-    const int L = F.len[b];
-    for (int i = 0; i < L; ++i) {
-        const C v = t[(long long)wrap_nonneg(2 * k + i, m) * n];
-        const R hi_ = g[i], lo_ = h[i];
-        lx += lo_ * v.x; ly += lo_ * v.y; hx += hi_ * v.x; hy += hi_ * v.y;
+    WL_SWITCH_L(b, (col_fwd_body<R, L>(t, d, n, m, k0, h, g)))
+}
+
+// ---- synthesis, one axis: 2 KPT consecutive samples j0 .. j0 + 2 KPT - 1 (j0 even) from the low / high coefficients
+// kk = kmin .. kmin + KPT + L/2 - 2, kmin = (j0 - (L - 2)) / 2:  out[j0 + jj] = sum h[i] lo[kk] + g[i] hi[kk], i = jj - 2 kr + L - 2
+template <typename R, int L, typename LoadLo, typename LoadHi, typename Store>
+__device__ __forceinline__ void inv_body(int mh, int j0, const R* __restrict__ h, const R* __restrict__ g, LoadLo load_lo, LoadHi load_hi,
+                                         Store store) {
+    typedef typename C2T<R>::type C;
+    R ax[2 * KPT], ay[2 * KPT];
+#pragma unroll
+    for (int jj = 0; jj < 2 * KPT; ++jj) ax[jj] = ay[jj] = (R)0;
+    int kk = wrap_any((j0 - (L - 2)) / 2, mh);                 // (j0 - L + 2 is even; C division of a negative even number is exact)
+#pragma unroll
+    for (int kr = 0; kr < KPT + L / 2 - 1; ++kr) {
+        const C lo = load_lo(kk), hi = load_hi(kk);
+        if (++kk == mh) kk = 0;
+#pragma unroll
+        for (int jj = 0; jj < 2 * KPT; ++jj) {
+            const int i = jj - 2 * kr + (L - 2);
+            if (i >= 0 && i < L) { ax[jj] += h[i] * lo.x + g[i] * hi.x; ay[jj] += h[i] * lo.y + g[i] * hi.y; }
+        }
     }
-    C* d = dst + (long long)b * dst_stride + c;
-    C lo; lo.x = lx; lo.y = ly;
-    C hi; hi.x = hx; hi.y = hy;
-    d[(long long)k * n] = lo;
-    d[(long long)(mh + k) * n] = hi;
+#pragma unroll
+    for (int jj = 0; jj < 2 * KPT; ++jj) { C o; o.x = ax[jj]; o.y = ay[jj]; store(jj, o); }
 }
 
 // ---- synthesis along y: the m x m block whose low-low quadrant comes from `ll` (the level below, already synthesised)
-// and whose other three quadrants come from `det` (the coefficients) -> tmp[b] rows j < m
+// and whose other three quadrants come from `det` (the coefficients) -> tmp[b] rows j < m.  Thread = one column.
 template <typename R>
 __global__ void __launch_bounds__(128) wl_col_inv(const typename C2T<R>::type* __restrict__ ll, long long ll_stride,
                                                   const typename C2T<R>::type* __restrict__ det, long long det_stride,
                                                   typename C2T<R>::type* __restrict__ tmp, long long tmp_stride, int n, int m,
-                                                  const R* __restrict__ filt, Filters F) {
+                                                  const R* __restrict__ filt) {
     typedef typename C2T<R>::type C;
-    const int c = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y, b = blockIdx.z, mh = m >> 1;
+    const int c = blockIdx.x * blockDim.x + threadIdx.x, j0 = blockIdx.y * 2 * KPT, b = blockIdx.z, mh = m >> 1;
     if (c >= m) return;
     const C* lo_src = (c < mh ? ll + (long long)b * ll_stride : det + (long long)b * det_stride) + c;     // rows [0, m/2)
-    const C* hi_src = det + (long long)b * det_stride + c;                                              // rows [m/2, m)
+    const C* hi_src = det + (long long)b * det_stride + (long long)mh * n + c;                          // rows [m/2, m)
+    C* out = tmp + (long long)b * tmp_stride + c;
     const R* h = filt + (b * 2) * LMAX;
     const R* g = h + LMAX;
-    R ax = 0, ay = 0;
-    const int L = F.len[b];
-    for (int i = j & 1; i < L; i += 2) {
-        const int kk = wrap_any((j - i) >> 1, mh);
-        const C lo = lo_src[(long long)kk * n], hi = hi_src[(long long)(mh + kk) * n];
-        ax += h[i] * lo.x + g[i] * hi.x;
-        ay += h[i] * lo.y + g[i] * hi.y;
-    }
-    C o; o.x = ax; o.y = ay;
-    tmp[(long long)b * tmp_stride + (long long)j * n + c] = o;
+    auto load_lo = [&](int kk) { return lo_src[(long long)kk * n]; };
+    auto load_hi = [&](int kk) { return hi_src[(long long)kk * n]; };
+    auto store = [&](int jj, C o) { if (j0 + jj < m) out[(long long)(j0 + jj) * n] = o; };
+    WL_SWITCH_L(b, (inv_body<R, L>(mh, j0, h, g, load_lo, load_hi, store)))
 }
 
-// ---- synthesis along x: tmp[b] (m x m block) -> out[b] (m x m block)
+// ---- synthesis along x: tmp[b] (m x m block) -> out[b] (m x m block).  Thread = 2 KPT consecutive samples of one row
+// (the shared-memory staging that pays for the analysis was measured slower here: 0.58 vs 0.31 ms for Psi at n = 2048).
 template <typename R>
 __global__ void __launch_bounds__(128) wl_row_inv(const typename C2T<R>::type* __restrict__ tmp, long long tmp_stride,
                                                   typename C2T<R>::type* __restrict__ out, long long out_stride, int n, int m,
-                                                  const R* __restrict__ filt, Filters F) {
+                                                  const R* __restrict__ filt) {
     typedef typename C2T<R>::type C;
-    const int j = blockIdx.x * blockDim.x + threadIdx.x, r = blockIdx.y, b = blockIdx.z, mh = m >> 1;
-    if (j >= m) return;
+    const int j0 = (blockIdx.x * blockDim.x + threadIdx.x) * 2 * KPT, r = blockIdx.y, b = blockIdx.z, mh = m >> 1;
+    if (j0 >= m) return;
     const C* t = tmp + (long long)b * tmp_stride + (long long)r * n;
+    C* o_ = out + (long long)b * out_stride + (long long)r * n;
     const R* h = filt + (b * 2) * LMAX;
     const R* g = h + LMAX;
-    R ax = 0, ay = 0;
-    const int L = F.len[b];
-    for (int i = j & 1; i < L; i += 2) {
-        const int kk = wrap_any((j - i) >> 1, mh);
-        const C lo = t[kk], hi = t[mh + kk];
-        ax += h[i] * lo.x + g[i] * hi.x;
-        ay += h[i] * lo.y + g[i] * hi.y;
-    }
-    C o; o.x = ax; o.y = ay;
-    out[(long long)b * out_stride + (long long)r * n + j] = o;
+    auto load_lo = [&](int kk) { return t[kk]; };
+    auto load_hi = [&](int kk) { return t[mh + kk]; };
+    auto store = [&](int jj, C o) { if (j0 + jj < m) o_[j0 + jj] = o; };
+    WL_SWITCH_L(b, (inv_body<R, L>(mh, j0, h, g, load_lo, load_hi, store)))
 }
 
 // ---- last synthesis pass (level 0, along x) of all eight bases + the Dirac coefficients, summed (Eq. 41), with the
-// epilogue: MODE 0: x = sum; MODE 1: zbar = P_C(z - sum) (Algorithm 1 line 13)
+// epilogue: MODE 0: x = sum; MODE 1: zbar = P_C(z - sum) (Algorithm 1 line 13).  Thread = 2 KPT consecutive samples.
 template <typename R, int MODE>
 __global__ void __launch_bounds__(128) wl_row_inv_sum(const typename C2T<R>::type* __restrict__ tmp, long long tmp_stride,
                                                       const typename C2T<R>::type* __restrict__ dirac,
                                                       const typename C2T<R>::type* __restrict__ z,
                                                       typename C2T<R>::type* __restrict__ out, int n,
-                                                      const R* __restrict__ filt, Filters F) {
+                                                      const R* __restrict__ filt) {
     typedef typename C2T<R>::type C;
-    const int j = blockIdx.x * blockDim.x + threadIdx.x, r = blockIdx.y, mh = n >> 1;
-    if (j >= n) return;
-    const C d0 = dirac[(long long)r * n + j];
-    R ax = d0.x, ay = d0.y;
+    const int j0 = (blockIdx.x * blockDim.x + threadIdx.x) * 2 * KPT, r = blockIdx.y, mh = n >> 1;
+    if (j0 >= n) return;
+    R sx[2 * KPT], sy[2 * KPT];
+#pragma unroll
+    for (int jj = 0; jj < 2 * KPT; ++jj) {
+        sx[jj] = sy[jj] = (R)0;
+        if (j0 + jj < n) { const C d0 = dirac[(long long)r * n + j0 + jj]; sx[jj] = d0.x; sy[jj] = d0.y; }
+    }
+    auto store = [&](int jj, C o) { sx[jj] += o.x; sy[jj] += o.y; };
+#pragma unroll 1
     for (int b = 0; b < NB; ++b) {
         const C* t = tmp + (long long)b * tmp_stride + (long long)r * n;
         const R* h = filt + (b * 2) * LMAX;
         const R* g = h + LMAX;
-        const int L = F.len[b];
-        for (int i = j & 1; i < L; i += 2) {
-            const int kk = wrap_any((j - i) >> 1, mh);
-            const C lo = t[kk], hi = t[mh + kk];
-            ax += h[i] * lo.x + g[i] * hi.x;
-            ay += h[i] * lo.y + g[i] * hi.y;
-        }
+        auto load_lo = [&](int kk) { return t[kk]; };
+        auto load_hi = [&](int kk) { return t[mh + kk]; };
+        WL_SWITCH_L(b, (inv_body<R, L>(mh, j0, h, g, load_lo, load_hi, store)))
     }
-    C o;
-    if (MODE == 0) { o.x = ax; o.y = ay; }
-    else { const C zz = z[(long long)r * n + j]; const R v = zz.x - ax; o.x = v > (R)0 ? v : (R)0; o.y = (R)0; }
-    out[(long long)r * n + j] = o;
+#pragma unroll
+    for (int jj = 0; jj < 2 * KPT; ++jj)
+        if (j0 + jj < n) {
+            C o;
+            if (MODE == 0) { o.x = sx[jj]; o.y = sy[jj]; }
+            else { const C zz = z[(long long)r * n + j0 + jj]; const R v = zz.x - sx[jj]; o.x = v > (R)0 ? v : (R)0; o.y = (R)0; }
+            out[(long long)r * n + j0 + jj] = o;
+        }
 }
 
 // ---- d <- (1/eta) (I - S_gamma)(eta d + a)   (Algorithm 1 line 12; Eq. 26 on the complex modulus)
@@ -275,8 +350,8 @@ int adjoint_t(purify_wavelet* w, const void* x, void* alpha, cudaStream_t st) {
     for (int lev = 0; lev < w->levels; ++lev) {
         const int m = n >> lev, mh = m >> 1;
         const C* src = lev == 0 ? (const C*)x : a;
-        wl_row_fwd<R><<<dim3((mh + 127) / 128, m, NB), 128, 0, st>>>(src, lev == 0 ? 0 : nn, n, (C*)w->tmp, nn, n, m, (const R*)w->filt, w->F);
-        wl_col_fwd<R><<<dim3((m + 127) / 128, mh, NB), 128, 0, st>>>((const C*)w->tmp, nn, a, nn, n, m, (const R*)w->filt, w->F);
+        wl_row_fwd<R><<<dim3((mh + ROW_SPAN - 1) / ROW_SPAN, m, NB), 128, 0, st>>>(src, lev == 0 ? 0 : nn, n, (C*)w->tmp, nn, n, m, (const R*)w->filt);
+        wl_col_fwd<R><<<dim3((m + 127) / 128, (mh + KPT - 1) / KPT, NB), 128, 0, st>>>((const C*)w->tmp, nn, a, nn, n, m, (const R*)w->filt);
         w->launches += 2;
     }
     WCK(cudaGetLastError());
@@ -294,12 +369,13 @@ int forward_t(purify_wavelet* w, const void* alpha, const void* z, void* out, cu
     for (int lev = w->levels - 1; lev >= 0; --lev) {
         const int m = n >> lev;
         const C* ll = lev == w->levels - 1 ? a : wk;          // the deepest level takes its low-low block from the coefficients
-        wl_col_inv<R><<<dim3((m + 127) / 128, m, NB), 128, 0, st>>>(ll, nn, a, nn, (C*)w->tmp, nn, n, m, (const R*)w->filt, w->F);
+        const int blk = (m + 2 * KPT - 1) / (2 * KPT);            // 2 KPT samples per thread along the blocked axis
+        wl_col_inv<R><<<dim3((m + 127) / 128, blk, NB), 128, 0, st>>>(ll, nn, a, nn, (C*)w->tmp, nn, n, m, (const R*)w->filt);
         if (lev > 0)
-            wl_row_inv<R><<<dim3((m + 127) / 128, m, NB), 128, 0, st>>>((const C*)w->tmp, nn, wk, nn, n, m, (const R*)w->filt, w->F);
+            wl_row_inv<R><<<dim3((blk + 127) / 128, m, NB), 128, 0, st>>>((const C*)w->tmp, nn, wk, nn, n, m, (const R*)w->filt);
         else
-            wl_row_inv_sum<R, MODE><<<dim3((n + 127) / 128, n), 128, 0, st>>>((const C*)w->tmp, nn, (const C*)alpha, (const C*)z, (C*)out, n,
-                                                                            (const R*)w->filt, w->F);
+            wl_row_inv_sum<R, MODE><<<dim3((blk + 127) / 128, n), 128, 0, st>>>((const C*)w->tmp, nn, (const C*)alpha, (const C*)z, (C*)out, n,
+                                                                              (const R*)w->filt);
         w->launches += 2;
     }
     WCK(cudaGetLastError());
