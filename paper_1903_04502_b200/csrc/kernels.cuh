@@ -306,6 +306,119 @@ __global__ void gather_from_native_kernel(const C* __restrict__ in, C* __restric
 }
 
 // ---------------------------------------------------------------------------------------------
+// Two-level permutation native <-> caller order (the caller-order entry points purify_degrid / purify_grid).
+// A single gather over M = 1e8 elements pays one DRAM access per 8-byte element.  Here the caller-order vector is cut
+// into TILES of PERM_TILE consecutive elements, and an intermediate order "mid" holds, tile after tile, the elements
+// of one caller tile in the order the native layout meets them:
+//   native -> mid   scatter with locality: the native order advances through every tile's segment front to back, so at
+//                   any moment only a few sectors per tile are open and L2 merges the 8-byte stores into full sectors;
+//   mid -> caller   a permutation INSIDE a tile, done in shared memory (coalesced loads and stores); in place.
+// and the reverse (caller -> mid in shared memory, mid -> native as a gather with the same locality).
+// Index arrays, built once at create: q[slot] = position in mid (0xFFFFFFFF for padding slots), loc[k] = position of
+// mid element k inside its caller tile (16 bit).
+constexpr int PERM_TILE_SHIFT = 12, PERM_TILE = 1 << PERM_TILE_SHIFT, PERM_THREADS = 512;
+
+__global__ void tile_key_kernel(const unsigned* __restrict__ perm, long long S, unsigned n_tiles,
+                                unsigned* __restrict__ keys, unsigned* __restrict__ vals) {
+    for (long long s = blockIdx.x * (long long)blockDim.x + threadIdx.x; s < S; s += (long long)gridDim.x * blockDim.x) {
+        const unsigned pi = perm[s];
+        keys[s] = pi == 0xFFFFFFFFu ? n_tiles : (pi >> PERM_TILE_SHIFT);     // padding slots sort behind the last tile
+        vals[s] = (unsigned)s;
+    }
+}
+// after the stable sort by tile: slot_of[k] is the native slot of mid element k (k < M)
+__global__ void two_level_fill_kernel(const unsigned* __restrict__ slot_of, const unsigned* __restrict__ perm, long long M,
+                                      unsigned* __restrict__ q, unsigned short* __restrict__ loc) {
+    for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < M; k += (long long)gridDim.x * blockDim.x) {
+        const unsigned s = slot_of[k];
+        q[s] = (unsigned)k;
+        loc[k] = (unsigned short)(perm[s] & (unsigned)(PERM_TILE - 1));
+    }
+}
+
+constexpr int MID_EPT = 8;      // elements per thread, loads issued together
+template <typename C>
+__global__ void __launch_bounds__(256) scatter_to_mid_kernel(const C* __restrict__ in, C* __restrict__ mid,
+                                                             const unsigned* __restrict__ q, long long S) {
+    const long long base = (long long)blockIdx.x * (256 * MID_EPT) + threadIdx.x;
+    unsigned qi[MID_EPT];
+    C v[MID_EPT];
+#pragma unroll
+    for (int e = 0; e < MID_EPT; ++e) {
+        const long long s = base + e * 256;
+        qi[e] = s < S ? q[s] : 0xFFFFFFFFu;
+        if (s < S) v[e] = in[s];
+    }
+#pragma unroll
+    for (int e = 0; e < MID_EPT; ++e)
+        if (qi[e] != 0xFFFFFFFFu) mid[qi[e]] = v[e];
+}
+template <typename C>
+__global__ void __launch_bounds__(256) gather_from_mid_kernel(const C* __restrict__ mid, C* __restrict__ out,
+                                                              const unsigned* __restrict__ q, long long S) {
+    const long long base = (long long)blockIdx.x * (256 * MID_EPT) + threadIdx.x;
+    unsigned qi[MID_EPT];
+    C v[MID_EPT];
+#pragma unroll
+    for (int e = 0; e < MID_EPT; ++e) {
+        const long long s = base + e * 256;
+        qi[e] = s < S ? q[s] : 0xFFFFFFFFu;
+    }
+#pragma unroll
+    for (int e = 0; e < MID_EPT; ++e) {
+        v[e].x = 0; v[e].y = 0;
+        if (qi[e] != 0xFFFFFFFFu) v[e] = mid[qi[e]];
+    }
+#pragma unroll
+    for (int e = 0; e < MID_EPT; ++e) {
+        const long long s = base + e * 256;
+        if (s < S) out[s] = v[e];
+    }
+}
+// one CTA per caller tile.  DIR 0: mid -> caller (out may be the same buffer as in), DIR 1: caller -> mid.
+template <typename C, int DIR>
+__global__ void __launch_bounds__(PERM_THREADS) tile_permute_kernel(const C* in, C* out, const unsigned short* __restrict__ loc,
+                                                                     long long M) {
+    extern __shared__ __align__(16) unsigned char perm_smem[];
+    C* tile = reinterpret_cast<C*>(perm_smem);
+    constexpr int EPT = PERM_TILE / PERM_THREADS;
+    const long long base = (long long)blockIdx.x * PERM_TILE;
+    const int n = (int)((M - base) < (long long)PERM_TILE ? (M - base) : (long long)PERM_TILE);
+    C v[EPT];
+    unsigned short l[EPT];
+#pragma unroll
+    for (int e = 0; e < EPT; ++e) {
+        const int j = threadIdx.x + e * PERM_THREADS;
+        if (j < n) { v[e] = in[base + j]; l[e] = loc[base + j]; }
+    }
+    if (DIR == 0) {
+#pragma unroll
+        for (int e = 0; e < EPT; ++e) {
+            const int j = threadIdx.x + e * PERM_THREADS;
+            if (j < n) tile[l[e]] = v[e];
+        }
+        __syncthreads();
+#pragma unroll
+        for (int e = 0; e < EPT; ++e) {
+            const int j = threadIdx.x + e * PERM_THREADS;
+            if (j < n) out[base + j] = tile[j];
+        }
+    } else {
+#pragma unroll
+        for (int e = 0; e < EPT; ++e) {
+            const int j = threadIdx.x + e * PERM_THREADS;
+            if (j < n) tile[j] = v[e];
+        }
+        __syncthreads();
+#pragma unroll
+        for (int e = 0; e < EPT; ++e) {
+            const int j = threadIdx.x + e * PERM_THREADS;
+            if (j < n) out[base + j] = tile[l[e]];
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
 // f2: pieces of the power method on Phi^dagger Phi.
 // sum of |x_i|^2 over a complex vector, accumulated in fp64 into *out (zeroed by the caller)
 template <typename R>

@@ -93,6 +93,12 @@ struct purify_op {
     void* w_s = nullptr;      // native-order weights
     unsigned* perm = nullptr; // native -> caller
     unsigned* inv_perm = nullptr; // caller -> native (batched layout)
+    // two-level permutation (kernels.cuh): position of every native slot in the tile-ordered intermediate vector, position
+    // of every intermediate element inside its caller tile; built at create when M >= TWO_LEVEL_MIN
+    unsigned* q_idx = nullptr;
+    unsigned short* loc_idx = nullptr;
+    void* perm_ws = nullptr;  // M complex: the intermediate vector of the caller -> native direction, lazily allocated
+    size_t perm_ws_bytes = 0;
     pk::Item* items = nullptr;
     void* corr = nullptr;     // s[n]
     void* table = nullptr;
@@ -447,9 +453,43 @@ int launch_fft(purify_op* op, int dir, cudaStream_t st) {
     return PURIFY_OK;
 }
 
+int ensure_ws(purify_op* op, void** p, size_t* have, size_t bytes);
+
+// below this many visibilities the permutation is L2-resident and one gather is cheaper than two passes
+constexpr long long TWO_LEVEL_MIN = 1ll << 22;
+
+template <typename C>
+int launch_permute_two_level(purify_op* op, const C* in, C* out, int to_native, cudaStream_t st) {
+    const long long M = op->M, S = op->M_native;
+    const unsigned n_tiles = (unsigned)((M + pk::PERM_TILE - 1) / pk::PERM_TILE);
+    const unsigned blocks = (unsigned)((S + 256 * pk::MID_EPT - 1) / (256 * pk::MID_EPT));
+    const size_t smem = sizeof(C) * pk::PERM_TILE;
+    static bool attr_done[2] = {false, false};
+    if (smem > 48 * 1024 && !attr_done[to_native]) {
+        if (to_native) CK(cudaFuncSetAttribute(pk::tile_permute_kernel<C, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        else CK(cudaFuncSetAttribute(pk::tile_permute_kernel<C, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_done[to_native] = true;
+    }
+    if (!to_native) {              // native -> mid (scatter with locality, into the caller's buffer) -> caller (in place, per tile)
+        pk::scatter_to_mid_kernel<C><<<blocks, 256, 0, st>>>(in, out, op->q_idx, S);
+        pk::tile_permute_kernel<C, 0><<<n_tiles, pk::PERM_THREADS, smem, st>>>(out, out, op->loc_idx, M);
+    } else {                       // caller -> mid (per tile, through shared memory) -> native (gather with locality)
+        int rc = ensure_ws(op, &op->perm_ws, &op->perm_ws_bytes, sizeof(C) * (size_t)M);
+        if (rc) return rc;
+        pk::tile_permute_kernel<C, 1><<<n_tiles, pk::PERM_THREADS, smem, st>>>(in, (C*)op->perm_ws, op->loc_idx, M);
+        pk::gather_from_mid_kernel<C><<<blocks, 256, 0, st>>>((const C*)op->perm_ws, out, op->q_idx, S);
+    }
+    op->launches += 2;
+    CK(cudaGetLastError());
+    return PURIFY_OK;
+}
+
 int launch_permute(purify_op* op, const void* in, void* out, int to_native, cudaStream_t st) {
     StageTimer t(op, PURIFY_STAGE_PERMUTE, st);
     if (op->M_native == 0) return PURIFY_OK;
+    if (op->q_idx && op->M > 0)
+        return op->dtype == PURIFY_C64 ? launch_permute_two_level<float2>(op, (const float2*)in, (float2*)out, to_native, st)
+                                       : launch_permute_two_level<double2>(op, (const double2*)in, (double2*)out, to_native, st);
     if (!to_native && op->inv_perm) {
         if (op->M > 0 && op->dtype == PURIFY_C64)
             pk::gather_from_native_kernel<float2><<<grid_for(op->M, 256, 148 * 32), 256, 0, st>>>((const float2*)in, (float2*)out, op->inv_perm, op->M);
@@ -767,7 +807,35 @@ int build_bins_x(purify_op* op, const void* uv_dev, const void* w_dev, cudaStrea
             op->perm, (F*)op->uv_s);
         CKC(cudaGetLastError());
     }
-    if (M > 0) {
+    if (M >= TWO_LEVEL_MIN) {
+        // index arrays of the two-level permutation: stable sort of the slots by caller tile (padding slots last)
+        const long long S = op->M_native;
+        const unsigned n_tiles = (unsigned)((M + pk::PERM_TILE - 1) / pk::PERM_TILE);
+        int bits = 1;
+        while ((1u << bits) <= n_tiles) ++bits;
+        unsigned *tk = nullptr, *tk2 = nullptr, *tv = nullptr, *tv2 = nullptr;
+        void* tmp2 = nullptr;
+        size_t tmp2_bytes = 0;
+        auto free_t = [&]() { cudaFree(tk); cudaFree(tk2); cudaFree(tv); cudaFree(tv2); cudaFree(tmp2); };
+        cudaError_t e = cudaMalloc(&tk, sizeof(unsigned) * S);
+        if (e == cudaSuccess) e = cudaMalloc(&tk2, sizeof(unsigned) * S);
+        if (e == cudaSuccess) e = cudaMalloc(&tv, sizeof(unsigned) * S);
+        if (e == cudaSuccess) e = cudaMalloc(&tv2, sizeof(unsigned) * S);
+        if (e == cudaSuccess) e = cub::DeviceRadixSort::SortPairs(nullptr, tmp2_bytes, tk, tk2, tv, tv2, (int)S, 0, bits, st);
+        if (e == cudaSuccess) e = cudaMalloc(&tmp2, tmp2_bytes ? tmp2_bytes : 16);
+        if (e != cudaSuccess) { cudaGetLastError(); free_t(); cleanup(); return fail(PURIFY_ERR_ALLOC, "two-level permutation: temporaries: %s", cudaGetErrorString(e)); }
+        if ((rc = dev_alloc(op, (void**)&op->q_idx, sizeof(unsigned) * (size_t)S)) ||
+            (rc = dev_alloc(op, (void**)&op->loc_idx, sizeof(unsigned short) * (size_t)M))) { free_t(); cleanup(); return rc; }
+        pk::tile_key_kernel<<<grid_for(S, 256), 256, 0, st>>>(op->perm, S, n_tiles, tk, tv);
+        e = cub::DeviceRadixSort::SortPairs(tmp2, tmp2_bytes, tk, tk2, tv, tv2, (int)S, 0, bits, st);
+        if (e == cudaSuccess) e = cudaMemsetAsync(op->q_idx, 0xFF, sizeof(unsigned) * (size_t)S, st);
+        if (e == cudaSuccess) {
+            pk::two_level_fill_kernel<<<grid_for(M, 256), 256, 0, st>>>(tv2, op->perm, M, op->q_idx, op->loc_idx);
+            e = cudaStreamSynchronize(st);
+        }
+        free_t();
+        CKC(e);
+    } else if (M > 0) {
         if ((rc = dev_alloc(op, (void**)&op->inv_perm, sizeof(unsigned) * (size_t)M))) { cleanup(); return rc; }
         pk::invert_perm_kernel<<<grid_for(op->M_native, 256), 256, 0, st>>>(op->perm, op->M_native, op->inv_perm);
         CKC(cudaGetLastError());
@@ -973,7 +1041,7 @@ int purify_op_create_host(purify_op** out, int n, int oversample, int J, long lo
 
 int purify_op_destroy(purify_op* op) {
     if (!op) return PURIFY_OK;
-    cudaFree(op->grid); cudaFree(op->uv_s); cudaFree(op->w_s); cudaFree(op->perm); cudaFree(op->inv_perm); cudaFree(op->scal_ws); cudaFree(op->items);
+    cudaFree(op->grid); cudaFree(op->uv_s); cudaFree(op->w_s); cudaFree(op->perm); cudaFree(op->inv_perm); cudaFree(op->q_idx); cudaFree(op->loc_idx); cudaFree(op->perm_ws); cudaFree(op->scal_ws); cudaFree(op->items);
     cudaFree(op->corr); cudaFree(op->table); cudaFree(op->y_ws); cudaFree(op->x_ws); cudaFree(op->y_ws2);
     cudaFree(op->x_bhdr); cudaFree(op->x_blane); cudaFree(op->x_items); cudaFree(op->x_counter);
     for (cudaEvent_t e : op->band_ev) cudaEventDestroy(e);

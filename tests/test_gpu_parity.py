@@ -518,3 +518,41 @@ def test_gridding_repeatable_under_stress_on_hot_cells():
         worst = max(worst, float((op.stage_gridded(yd) - first).abs().max()) / scale)
     assert worst <= 2e-6, worst                              # reduction order varies (atomics at L2): rounding only
     op.close()
+
+
+@pytest.mark.parametrize("dtype", ["c64", "c128"])
+def test_two_level_permutation_is_the_permutation(dtype):
+    """Above 2^22 visibilities the caller-order entry points permute in two passes (caller tiles of 4096 elements through
+    shared memory + a pass with locality through an intermediate order, kernels.cuh).  Index work: bit-exact against
+    purify_op_permutation, both directions, at a ragged size (last caller tile and last 2048-slot block partial), with
+    NaN canaries around the outputs."""
+    from paper_1903_04502_b200 import C64, C128, PurifyOp
+    M = (1 << 22) + 1234
+    rng = np.random.default_rng(77)
+    K = 512
+    uv = rng.normal(0.0, K / 6, size=(M, 2)).clip(-K / 2 + 9, K / 2 - 9).astype(synth.real_dtype(dtype))
+    op = PurifyOp(256, 4, torch.from_numpy(uv).cuda(), None, dtype=C64 if dtype == "c64" else C128)
+    perm = op.permutation().cpu().numpy()
+    Mn = op.M_native
+    cd = synth.complex_dtype(dtype)
+    real = perm >= 0
+    assert real.sum() == M and np.array_equal(np.sort(perm[real]), np.arange(M))
+    # native -> caller
+    v_nat = synth.random_complex((Mn,), seed=5, dtype=dtype)
+    buf = torch.full((M + 64,), complex(float("nan"), float("nan")), dtype=torch.from_numpy(v_nat).dtype, device="cuda")
+    out = op.permute_from_native(torch.from_numpy(v_nat).cuda(), out=buf[32:32 + M])
+    ref = np.empty(M, dtype=cd)
+    ref[perm[real]] = v_nat[real]
+    assert np.array_equal(out.cpu().numpy().view(np.uint8), ref.view(np.uint8))
+    flank = torch.cat([buf[:32], buf[32 + M:]]).cpu().numpy()
+    assert np.isnan(flank.real).all() and np.isnan(flank.imag).all()
+    # caller -> native (padding slots become 0)
+    v_call = synth.random_complex((M,), seed=6, dtype=dtype)
+    buf2 = torch.full((Mn + 64,), complex(float("nan"), float("nan")), dtype=buf.dtype, device="cuda")
+    out2 = op.permute_to_native(torch.from_numpy(v_call).cuda(), out=buf2[32:32 + Mn])
+    ref2 = np.zeros(Mn, dtype=cd)
+    ref2[real] = v_call[perm[real]]
+    assert np.array_equal(out2.cpu().numpy().view(np.uint8), ref2.view(np.uint8))
+    flank2 = torch.cat([buf2[:32], buf2[32 + Mn:]]).cpu().numpy()
+    assert np.isnan(flank2.real).all() and np.isnan(flank2.imag).all()
+    op.close()
