@@ -137,6 +137,11 @@ int purify_normal(purify_op *op, const void *x_in_dev, void *x_out_dev, void *cu
  * 16-byte aligned (INVALID_ARG otherwise: the kernel streams it with bulk copies). */
 int purify_degrid_native(purify_op *op, const void *x_dev, void *y_native_dev, void *cuda_stream);
 int purify_grid_native(purify_op *op, const void *y_native_dev, void *x_dev, void *cuda_stream);
+/* The permutation passes on their own (also what purify_degrid / purify_grid run after / before the native kernels).
+ * Input and output must not overlap.  From 2^24 visibilities on the permutation is routed in three coalesced passes
+ * (blocks permuted in shared memory, runs of consecutive elements written: native order -> grouped by ranges of the
+ * caller index -> grouped by caller tiles of 4096 -> caller order; index arrays built at create) and the handle
+ * lazily allocates M (from native) or 2 M (to native) complex entries of workspace; below, one gather. */
 int purify_permute_to_native(purify_op *op, const void *y_caller_dev, void *y_native_dev, void *cuda_stream);
 int purify_permute_from_native(purify_op *op, const void *y_native_dev, void *y_caller_dev, void *cuda_stream);
 

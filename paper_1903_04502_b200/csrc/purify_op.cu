@@ -93,11 +93,13 @@ struct purify_op {
     void* w_s = nullptr;      // native-order weights
     unsigned* perm = nullptr; // native -> caller
     unsigned* inv_perm = nullptr; // caller -> native (batched layout)
-    // two-level permutation (kernels.cuh): position of every native slot in the tile-ordered intermediate vector, position
-    // of every intermediate element inside its caller tile; built at create when M >= TWO_LEVEL_MIN
-    unsigned* q_idx = nullptr;
-    unsigned short* loc_idx = nullptr;
-    void* perm_ws = nullptr;  // M complex: the intermediate vector of the caller -> native direction, lazily allocated
+    // routed permutation (kernels.cuh), index arrays built at create when M >= ROUTED_MIN
+    unsigned short* loc_a = nullptr;   // pass A: rank of every native slot inside its block (NONE16: padding)
+    unsigned* dst_a = nullptr;         //         A-order position of every sorted rank
+    unsigned short* loc_b = nullptr;   // pass B: rank of every A-order element inside its block
+    unsigned* dst_b = nullptr;         //         mid position of every sorted rank
+    unsigned short* loc_idx = nullptr; // pass C: position of every mid element inside its caller tile
+    void* perm_ws = nullptr;           // intermediate vectors (M complex from native, 2 M complex to native), lazily allocated
     size_t perm_ws_bytes = 0;
     pk::Item* items = nullptr;
     void* corr = nullptr;     // s[n]
@@ -455,31 +457,39 @@ int launch_fft(purify_op* op, int dir, cudaStream_t st) {
 
 int ensure_ws(purify_op* op, void** p, size_t* have, size_t bytes);
 
-// below this many visibilities the permutation is L2-resident and one gather is cheaper than two passes
-constexpr long long TWO_LEVEL_MIN = 1ll << 22;
+// below this many visibilities the permutation is L2-resident and one gather is cheaper than three passes
+constexpr long long ROUTED_MIN = 1ll << 24;   // (measured: 1e7 elements 0.065 ms by one gather against 0.125 ms routed; 1e8: 2.16 against 1.07 ms)
+// block size of the routing passes: 2^13 complex64 / 2^12 complex128 elements = 64 KB of shared memory
+inline int route_bs(const purify_op* op) { return op->dtype == PURIFY_C64 ? 13 : 12; }
 
-template <typename C>
-int launch_permute_two_level(purify_op* op, const C* in, C* out, int to_native, cudaStream_t st) {
+template <typename C, int BS>
+int launch_permute_routed(purify_op* op, const C* in, C* out, int to_native, cudaStream_t st) {
     const long long M = op->M, S = op->M_native;
     const unsigned n_tiles = (unsigned)((M + pk::PERM_TILE - 1) / pk::PERM_TILE);
-    const unsigned blocks = (unsigned)((S + 256 * pk::MID_EPT - 1) / (256 * pk::MID_EPT));
-    const size_t smem = sizeof(C) * pk::PERM_TILE;
-    static bool attr_done[2] = {false, false};
-    if (smem > 48 * 1024 && !attr_done[to_native]) {
-        if (to_native) CK(cudaFuncSetAttribute(pk::tile_permute_kernel<C, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        else CK(cudaFuncSetAttribute(pk::tile_permute_kernel<C, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_done[to_native] = true;
+    const unsigned blocks_a = (unsigned)((S + (1ll << BS) - 1) >> BS), blocks_b = (unsigned)((M + (1ll << BS) - 1) >> BS);
+    const size_t smem_r = sizeof(C) << BS, smem_t = sizeof(C) * pk::PERM_TILE;
+    static bool attr_done = false;
+    if (!attr_done) {
+        CK(cudaFuncSetAttribute(pk::route_kernel<C, BS, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_r));
+        CK(cudaFuncSetAttribute(pk::route_kernel<C, BS, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_r));
+        CK(cudaFuncSetAttribute(pk::tile_permute_kernel<C, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_t));
+        CK(cudaFuncSetAttribute(pk::tile_permute_kernel<C, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_t));
+        attr_done = true;
     }
-    if (!to_native) {              // native -> mid (scatter with locality, into the caller's buffer) -> caller (in place, per tile)
-        pk::scatter_to_mid_kernel<C><<<blocks, 256, 0, st>>>(in, out, op->q_idx, S);
-        pk::tile_permute_kernel<C, 0><<<n_tiles, pk::PERM_THREADS, smem, st>>>(out, out, op->loc_idx, M);
-    } else {                       // caller -> mid (per tile, through shared memory) -> native (gather with locality)
-        int rc = ensure_ws(op, &op->perm_ws, &op->perm_ws_bytes, sizeof(C) * (size_t)M);
-        if (rc) return rc;
-        pk::tile_permute_kernel<C, 1><<<n_tiles, pk::PERM_THREADS, smem, st>>>(in, (C*)op->perm_ws, op->loc_idx, M);
-        pk::gather_from_mid_kernel<C><<<blocks, 256, 0, st>>>((const C*)op->perm_ws, out, op->q_idx, S);
+    int rc = ensure_ws(op, &op->perm_ws, &op->perm_ws_bytes, sizeof(C) * (size_t)M * (to_native ? 2 : 1));
+    if (rc) return rc;
+    C* w0 = (C*)op->perm_ws;
+    C* w1 = w0 + M;
+    if (!to_native) {              // native -> A order -> mid (in the caller's buffer) -> caller order (in place)
+        pk::route_kernel<C, BS, 0><<<blocks_a, pk::PERM_THREADS, smem_r, st>>>(in, w0, op->loc_a, op->dst_a, S);
+        pk::route_kernel<C, BS, 0><<<blocks_b, pk::PERM_THREADS, smem_r, st>>>(w0, out, op->loc_b, op->dst_b, M);
+        pk::tile_permute_kernel<C, 0><<<n_tiles, pk::PERM_THREADS, smem_t, st>>>(out, out, op->loc_idx, M);
+    } else {                       // caller order -> mid -> A order -> native (padding slots: 0)
+        pk::tile_permute_kernel<C, 1><<<n_tiles, pk::PERM_THREADS, smem_t, st>>>(in, w0, op->loc_idx, M);
+        pk::route_kernel<C, BS, 1><<<blocks_b, pk::PERM_THREADS, smem_r, st>>>(w0, w1, op->loc_b, op->dst_b, M);
+        pk::route_kernel<C, BS, 1><<<blocks_a, pk::PERM_THREADS, smem_r, st>>>(w1, out, op->loc_a, op->dst_a, S);
     }
-    op->launches += 2;
+    op->launches += 3;
     CK(cudaGetLastError());
     return PURIFY_OK;
 }
@@ -487,9 +497,9 @@ int launch_permute_two_level(purify_op* op, const C* in, C* out, int to_native, 
 int launch_permute(purify_op* op, const void* in, void* out, int to_native, cudaStream_t st) {
     StageTimer t(op, PURIFY_STAGE_PERMUTE, st);
     if (op->M_native == 0) return PURIFY_OK;
-    if (op->q_idx && op->M > 0)
-        return op->dtype == PURIFY_C64 ? launch_permute_two_level<float2>(op, (const float2*)in, (float2*)out, to_native, st)
-                                       : launch_permute_two_level<double2>(op, (const double2*)in, (double2*)out, to_native, st);
+    if (op->loc_a && op->M > 0)
+        return op->dtype == PURIFY_C64 ? launch_permute_routed<float2, 13>(op, (const float2*)in, (float2*)out, to_native, st)
+                                       : launch_permute_routed<double2, 12>(op, (const double2*)in, (double2*)out, to_native, st);
     if (!to_native && op->inv_perm) {
         if (op->M > 0 && op->dtype == PURIFY_C64)
             pk::gather_from_native_kernel<float2><<<grid_for(op->M, 256, 148 * 32), 256, 0, st>>>((const float2*)in, (float2*)out, op->inv_perm, op->M);
@@ -807,32 +817,62 @@ int build_bins_x(purify_op* op, const void* uv_dev, const void* w_dev, cudaStrea
             op->perm, (F*)op->uv_s);
         CKC(cudaGetLastError());
     }
-    if (M >= TWO_LEVEL_MIN) {
-        // index arrays of the two-level permutation: stable sort of the slots by caller tile (padding slots last)
+    if (M >= ROUTED_MIN) {
+        // index arrays of the routed permutation (kernels.cuh): four stable radix sorts over the slots
         const long long S = op->M_native;
+        const int bs = route_bs(op);
         const unsigned n_tiles = (unsigned)((M + pk::PERM_TILE - 1) / pk::PERM_TILE);
-        int bits = 1;
-        while ((1u << bits) <= n_tiles) ++bits;
-        unsigned *tk = nullptr, *tk2 = nullptr, *tv = nullptr, *tv2 = nullptr;
+        int cs = pk::PERM_TILE_SHIFT + 3;                 // coarse bucket = 2^cs caller indices: at most 256 buckets, at least 8 tiles
+        while (((M - 1) >> cs) >= 256) ++cs;
+        const int kb = cs - pk::PERM_TILE_SHIFT + 1;
+        auto nbits = [](unsigned long long v) { int b = 1; while ((1ull << b) <= v) ++b; return b; };
+        unsigned *tk = nullptr, *tk2 = nullptr, *tv = nullptr, *tv2 = nullptr, *apos = nullptr, *slot_a = nullptr, *q = nullptr;
         void* tmp2 = nullptr;
         size_t tmp2_bytes = 0;
-        auto free_t = [&]() { cudaFree(tk); cudaFree(tk2); cudaFree(tv); cudaFree(tv2); cudaFree(tmp2); };
+        auto free_t = [&]() { cudaFree(tk); cudaFree(tk2); cudaFree(tv); cudaFree(tv2); cudaFree(apos); cudaFree(slot_a); cudaFree(q); cudaFree(tmp2); };
         cudaError_t e = cudaMalloc(&tk, sizeof(unsigned) * S);
         if (e == cudaSuccess) e = cudaMalloc(&tk2, sizeof(unsigned) * S);
         if (e == cudaSuccess) e = cudaMalloc(&tv, sizeof(unsigned) * S);
         if (e == cudaSuccess) e = cudaMalloc(&tv2, sizeof(unsigned) * S);
-        if (e == cudaSuccess) e = cub::DeviceRadixSort::SortPairs(nullptr, tmp2_bytes, tk, tk2, tv, tv2, (int)S, 0, bits, st);
+        if (e == cudaSuccess) e = cudaMalloc(&apos, sizeof(unsigned) * S);
+        if (e == cudaSuccess) e = cudaMalloc(&q, sizeof(unsigned) * S);
+        if (e == cudaSuccess) e = cudaMalloc(&slot_a, sizeof(unsigned) * (size_t)M);
+        if (e == cudaSuccess) e = cub::DeviceRadixSort::SortPairs(nullptr, tmp2_bytes, tk, tk2, tv, tv2, (int)S, 0, 32, st);
         if (e == cudaSuccess) e = cudaMalloc(&tmp2, tmp2_bytes ? tmp2_bytes : 16);
-        if (e != cudaSuccess) { cudaGetLastError(); free_t(); cleanup(); return fail(PURIFY_ERR_ALLOC, "two-level permutation: temporaries: %s", cudaGetErrorString(e)); }
-        if ((rc = dev_alloc(op, (void**)&op->q_idx, sizeof(unsigned) * (size_t)S)) ||
+        if (e != cudaSuccess) { cudaGetLastError(); free_t(); cleanup(); return fail(PURIFY_ERR_ALLOC, "routed permutation: temporaries: %s", cudaGetErrorString(e)); }
+        if ((rc = dev_alloc(op, (void**)&op->loc_a, sizeof(unsigned short) * (size_t)S)) ||
+            (rc = dev_alloc(op, (void**)&op->dst_a, sizeof(unsigned) * (size_t)S)) ||
+            (rc = dev_alloc(op, (void**)&op->loc_b, sizeof(unsigned short) * (size_t)M)) ||
+            (rc = dev_alloc(op, (void**)&op->dst_b, sizeof(unsigned) * (size_t)M)) ||
             (rc = dev_alloc(op, (void**)&op->loc_idx, sizeof(unsigned short) * (size_t)M))) { free_t(); cleanup(); return rc; }
-        pk::tile_key_kernel<<<grid_for(S, 256), 256, 0, st>>>(op->perm, S, n_tiles, tk, tv);
-        e = cub::DeviceRadixSort::SortPairs(tmp2, tmp2_bytes, tk, tk2, tv, tv2, (int)S, 0, bits, st);
-        if (e == cudaSuccess) e = cudaMemsetAsync(op->q_idx, 0xFF, sizeof(unsigned) * (size_t)S, st);
+        const int g1 = grid_for(S, 256), gm = grid_for(M, 256);
+        // (1) mid order: by caller tile; q[slot] = mid position, loc_idx = position inside the tile
+        pk::tile_key_kernel<<<g1, 256, 0, st>>>(op->perm, S, n_tiles, tk, tv);
+        e = cub::DeviceRadixSort::SortPairs(tmp2, tmp2_bytes, tk, tk2, tv, tv2, (int)S, 0, nbits(n_tiles), st);
         if (e == cudaSuccess) {
-            pk::two_level_fill_kernel<<<grid_for(M, 256), 256, 0, st>>>(tv2, op->perm, M, op->q_idx, op->loc_idx);
+            pk::mid_fill_kernel<<<gm, 256, 0, st>>>(tv2, op->perm, M, q, op->loc_idx);
+            // (2) A order: by coarse bucket; apos[slot] = A position, slot_a[k] = slot of A element k
+            pk::coarse_key_kernel<<<g1, 256, 0, st>>>(op->perm, S, cs, bs, 0, tk, tv);
+            e = cub::DeviceRadixSort::SortPairs(tmp2, tmp2_bytes, tk, tk2, tv, tv2, (int)S, 0, 9, st);
+        }
+        if (e == cudaSuccess) e = cudaMemcpyAsync(slot_a, tv2, sizeof(unsigned) * (size_t)M, cudaMemcpyDeviceToDevice, st);
+        if (e == cudaSuccess) {
+            pk::a_pos_kernel<<<gm, 256, 0, st>>>(slot_a, M, apos);
+            // (3) pass A: order inside every native block by bucket
+            pk::coarse_key_kernel<<<g1, 256, 0, st>>>(op->perm, S, cs, bs, 1, tk, tv);
+            e = cub::DeviceRadixSort::SortPairs(tmp2, tmp2_bytes, tk, tk2, tv, tv2, (int)S, 0, 9 + nbits((unsigned long long)((S - 1) >> bs)), st);
+        }
+        if (e == cudaSuccess) {
+            pk::pass_a_fill_kernel<<<g1, 256, 0, st>>>(tv2, op->perm, apos, S, bs, op->loc_a, op->dst_a);
+            // (4) pass B: order inside every A block by tile
+            pk::pass_b_key_kernel<<<gm, 256, 0, st>>>(slot_a, op->perm, M, cs, bs, kb, tk, tv);
+            e = cub::DeviceRadixSort::SortPairs(tmp2, tmp2_bytes, tk, tk2, tv, tv2, (int)M, 0, kb + nbits((unsigned long long)((M - 1) >> bs)), st);
+        }
+        if (e == cudaSuccess) {
+            pk::pass_b_fill_kernel<<<gm, 256, 0, st>>>(tv2, slot_a, q, M, bs, op->loc_b, op->dst_b);
             e = cudaStreamSynchronize(st);
         }
+        if (e == cudaSuccess) e = cudaGetLastError();
         free_t();
         CKC(e);
     } else if (M > 0) {
@@ -1041,7 +1081,7 @@ int purify_op_create_host(purify_op** out, int n, int oversample, int J, long lo
 
 int purify_op_destroy(purify_op* op) {
     if (!op) return PURIFY_OK;
-    cudaFree(op->grid); cudaFree(op->uv_s); cudaFree(op->w_s); cudaFree(op->perm); cudaFree(op->inv_perm); cudaFree(op->q_idx); cudaFree(op->loc_idx); cudaFree(op->perm_ws); cudaFree(op->scal_ws); cudaFree(op->items);
+    cudaFree(op->grid); cudaFree(op->uv_s); cudaFree(op->w_s); cudaFree(op->perm); cudaFree(op->inv_perm); cudaFree(op->loc_a); cudaFree(op->dst_a); cudaFree(op->loc_b); cudaFree(op->dst_b); cudaFree(op->loc_idx); cudaFree(op->perm_ws); cudaFree(op->scal_ws); cudaFree(op->items);
     cudaFree(op->corr); cudaFree(op->table); cudaFree(op->y_ws); cudaFree(op->x_ws); cudaFree(op->y_ws2);
     cudaFree(op->x_bhdr); cudaFree(op->x_blane); cudaFree(op->x_items); cudaFree(op->x_counter);
     for (cudaEvent_t e : op->band_ev) cudaEventDestroy(e);

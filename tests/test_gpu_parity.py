@@ -521,13 +521,13 @@ def test_gridding_repeatable_under_stress_on_hot_cells():
 
 
 @pytest.mark.parametrize("dtype", ["c64", "c128"])
-def test_two_level_permutation_is_the_permutation(dtype):
-    """Above 2^22 visibilities the caller-order entry points permute in two passes (caller tiles of 4096 elements through
-    shared memory + a pass with locality through an intermediate order, kernels.cuh).  Index work: bit-exact against
-    purify_op_permutation, both directions, at a ragged size (last caller tile and last 2048-slot block partial), with
-    NaN canaries around the outputs."""
+def test_routed_permutation_is_the_permutation(dtype):
+    """From 2^24 visibilities on the caller-order entry points permute in three routed passes (blocks of 8192 / 4096
+    elements permuted in shared memory, runs written to coarse buckets, then to caller tiles of 4096, then inside the
+    tile; kernels.cuh).  Index work: bit-exact against purify_op_permutation, both directions, at a ragged size (last
+    block, last coarse bucket and last caller tile partial), with NaN canaries around the outputs."""
     from paper_1903_04502_b200 import C64, C128, PurifyOp
-    M = (1 << 22) + 1234
+    M = (1 << 24) + 1234
     rng = np.random.default_rng(77)
     K = 512
     uv = rng.normal(0.0, K / 6, size=(M, 2)).clip(-K / 2 + 9, K / 2 - 9).astype(synth.real_dtype(dtype))
