@@ -4,6 +4,7 @@ Phi^dagger at M = 1e8 on one B200; % of HBM roofline).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 4] [--M m]
                     [--dtype c64|c128] [--order generated|shuffled] [--scaling weak|strong] [--ubench]
+                    [--kernel-mode analytic|table] [--table-R r]
 
 A "step" is one pass of the whole hot path, Phi^dagger Phi (S+Z, F, W G, G^dagger W^dagger,
 F^dagger, Z^dagger S^dagger) over the config's visibility set.  For N > 1 the paper's
@@ -49,6 +50,9 @@ def parse():
     ap.add_argument("--dtype", default="", choices=["", "c64", "c128"], help="override the config's dtype (config 3: both)")
     ap.add_argument("--order", default="generated", choices=["generated", "shuffled"],
                     help="order of the visibilities handed to create (config 3: time-ordered and shuffled)")
+    ap.add_argument("--kernel-mode", default="", choices=["", "analytic", "table"],
+                    help="override the config's kernel weights: analytic polynomial or the paper's pre-sampled table (PAPER.md:580-592)")
+    ap.add_argument("--table-R", type=int, default=0, help="table samples per unit with --kernel-mode table (default: the config's, 4096)")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"])
     ap.add_argument("--cpu-sample", type=int, default=4_000_000, help="visibilities in the oracle sample (--impl reference; M > 1e8)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -166,7 +170,11 @@ def effective_config(args):
     import dataclasses
     from inputs import synth
     cfg = synth.CONFIGS[args.config]
-    return dataclasses.replace(cfg, J=args.J) if args.J else cfg
+    if args.J:
+        cfg = dataclasses.replace(cfg, J=args.J)
+    if args.kernel_mode:
+        cfg = dataclasses.replace(cfg, kernel_mode=args.kernel_mode, table_R=args.table_R or cfg.table_R)
+    return cfg
 
 
 def run_reference(args):
